@@ -1,0 +1,142 @@
+/*
+ * rfa.h -- C ABI of librfa.so: explicit finite-difference stepping of the simplified bioheat
+ * equation of arXiv 1907.05709 (Kath, Handels, Mastmeyer) on a labelled voxel volume, on one
+ * NVIDIA B200 (sm_100a).  Plain pointers and sizes only; no C++ or torch types cross this boundary.
+ *
+ * What one time step computes (citations: line numbers of the paper text, PAPER.md):
+ *   for every voxel v = (i,j,k) of every scenario
+ *     held voxel (vessel / fixed label / Dirichlet needle voxel):   T^{n+1} = T^n       Eq. 13 :122-125, Alg. 1 :313
+ *     otherwise  T^{n+1} = T^n + dt/(rho c_p) * [ K * ( d2x + d2y + d2z )               Eq. 12 :117
+ *                                  + w_b c_b (T_a - T^n) + Q_m (+ Q in POWER voxels) ]   Eq. 9  :102
+ *       d2x = (T_{i-1} - 2 T_i + T_{i+1}) / dx^2  etc.                                   Eq. 11 :112
+ *       rho, c_p, K, w_b c_b, Q_m looked up from the voxel's label ("voxel-wise", :120)
+ *       outer grid faces: zero flux, the missing neighbour is the voxel itself (R-7)
+ *     necrosis[v] |= (T^{n+1} >= 60 C), sticky                                           :37, R-11/R-12
+ *   two temperature buffers are ping-ponged (Alg. 2 :321-337).
+ *
+ * Layout: every volume is x fastest, idx = i + nx*(j + ny*k); batched volumes are scenario-major.
+ * Arithmetic: fp32 on the device, stored as theta = T - t_blood (exact shift of the affine PDE,
+ * DESIGN.md section 5); per-label coefficients are derived in fp64 on the host and rounded once.
+ *
+ * Memory: "host" pointers are ordinary host memory.  Pointers documented "host or device" may be
+ * either (the library asks the CUDA runtime).  The library copies what it is given during the call;
+ * the caller keeps ownership of all its buffers.  Device state lives in the caller's workspace
+ * (see rfa_workspace_bytes) or, if none is given, in memory the library allocates and frees.
+ *
+ * Errors: every int-returning call returns RFA_OK (0) or a negative code; no exception crosses the
+ * ABI and a failed rfa_create leaves nothing allocated.  rfa_last_error() gives the message of the
+ * calling thread's last failure.  rfa_step is asynchronous on the simulation's stream; the rfa_get_*,
+ * rfa_necrotic_voxels and rfa_synchronize calls wait for it.
+ */
+#ifndef RFA_H
+#define RFA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rfa_sim rfa_sim; /* opaque */
+
+/* One row per label id, SI units (constants of PAPER.md:104). 28 bytes, no padding. */
+typedef struct rfa_tissue {
+    float k;        /* W/(m K)    thermal conductivity K                                    */
+    float rho;      /* kg/m^3     tissue density                                            */
+    float cp;       /* J/(kg K)   tissue heat capacity c_p                                  */
+    float wb_cb;    /* W/(m^3 K)  perfusion sink coefficient  w_b * c_b  of Eq. 9           */
+    float q_m;      /* W/m^3      metabolic heat Q_m                                        */
+    float t_init;   /* deg C      initial temperature of this label (Fig. 5)  */
+    uint32_t flags; /* RFA_TISSUE_HELD: never updated, stays at its temperature (Eq. 13)    */
+} rfa_tissue;
+
+enum { RFA_TISSUE_HELD = 1 };
+enum { RFA_MAX_TISSUES = 32 };   /* label ids 0..31 (5 bits of the packed state byte) */
+
+/* needle source modes (PAPER.md:145 held tip; BASELINE.json config 3 constant power, R-17) */
+enum { RFA_SRC_OFF = 0, RFA_SRC_DIRICHLET = 1 /* value = deg C */, RFA_SRC_POWER = 2 /* value = W/m^3 */ };
+
+enum {
+    RFA_OK = 0,
+    RFA_E_INVALID = -1,   /* null pointer, non-positive dims/spacing/dt, label >= n_tissue, > 32 tissues,
+                             scenario out of range, bad mode, workspace too small, non-finite constants */
+    RFA_E_UNSTABLE = -2,  /* dt violates the monotone bound dt*(2 alpha sum 1/h^2 + w_b c_b/(rho c_p)) <= 1
+                             for some non-held label (R-18)                                    */
+    RFA_E_CUDA = -3,      /* a CUDA runtime call or kernel launch failed (also: no device)              */
+    RFA_E_NOMEM = -4      /* host or device allocation failed                                          */
+};
+
+/* kernel variants for rfa_configure (all produce bit-identical fields) */
+enum {
+    RFA_KERNEL_AUTO = 0,      /* temporally blocked kernel where the grid allows it, else the plain one */
+    RFA_KERNEL_PLAIN = 1,     /* one thread per voxel, one step per launch, global loads only          */
+    RFA_KERNEL_BLOCKED = 2    /* 2.5D z-sweep with register queues, fused_steps time steps per launch   */
+};
+
+/* Bytes of device workspace rfa_create needs for these dims (nx,ny,nz) and batch; 0 on bad input. */
+size_t rfa_workspace_bytes(const int dims[3], int batch);
+
+/* Monotone stability number  max over non-held labels of  dt*(2 K/(rho c_p) (1/dx^2+1/dy^2+1/dz^2)
+ * + w_b c_b/(rho c_p));  rfa_create rejects values > 1 (R-18).  Host only, no GPU needed.
+ * Returns a negative value on invalid input. */
+double rfa_stability_number(const float spacing_mm[3], const rfa_tissue *table, int n_tissue, float dt_s);
+
+/* Create a simulation of `batch` independent scenarios that share one label volume.
+ *   dims        nx, ny, nz (> 0)
+ *   spacing_mm  voxel spacing in millimetres, converted to metres internally
+ *   labels      host, nx*ny*nz bytes, label ids < n_tissue
+ *   table       host, n_tissue rows (<= RFA_MAX_TISSUES)
+ *   t_blood_c   T_a of Eq. 9 (deg C); dt_s the time step (s)
+ *   workspace   device memory of >= rfa_workspace_bytes(dims,batch) bytes, 256-byte aligned, owned by
+ *               the caller and kept alive until rfa_destroy; or NULL (the library allocates)
+ *   cuda_stream a cudaStream_t (NULL = default stream); all work of this simulation runs on it
+ * Initial state: T = t_init of the label, no needle, necrosis = (T >= 60). */
+int rfa_create(rfa_sim **out, const int dims[3], const float spacing_mm[3], const uint8_t *labels,
+               const rfa_tissue *table, int n_tissue, float t_blood_c, float dt_s, int batch,
+               void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Place (or move, or with RFA_SRC_OFF remove) the needle of one scenario.
+ *   tip_mm, axis  metadata only, validated for finiteness (the mask is authoritative); may be NULL
+ *   mask          host or device, nx*ny*nz bytes, nonzero = electrode voxel; ignored for RFA_SRC_OFF
+ *   DIRICHLET: mask voxels are set to `value` deg C and held, overriding the label (R-15)
+ *   POWER:     mask voxels get +value W/m^3 in the bracket of Eq. 12; a held label stays held (R-17)
+ * Voxels of a previous needle are released: they keep their temperature and follow their label (R-16). */
+int rfa_set_needle(rfa_sim *s, int scenario, const float tip_mm[3], const float axis[3],
+                   const uint8_t *mask, int mode, float value);
+
+/* Overwrite the temperature image of one scenario (deg C, host or device, nx*ny*nz floats);
+ * necrosis |= (T >= 60).  Held voxels keep whatever is written here. */
+int rfa_set_temperature(rfa_sim *s, int scenario, const float *t_c);
+
+/* Advance every scenario by n time steps (n >= 0).  Asynchronous. */
+int rfa_step(rfa_sim *s, int n);
+
+/* Current temperature image (deg C) / necrosis mask (0 or 1) of one scenario into `out`
+ * (host or device, nx*ny*nz elements). */
+int rfa_get_temperature(rfa_sim *s, int scenario, float *out);
+int rfa_get_necrosis(rfa_sim *s, int scenario, uint8_t *out);
+
+/* Necrotic voxel counts of one scenario: all voxels of the mask, and those that are neither needle
+ * voxels nor held labels (the reported necrotic volume, R-13).  Either pointer may be NULL. */
+int rfa_necrotic_voxels(rfa_sim *s, int scenario, int64_t *all_voxels, int64_t *tissue_voxels);
+
+/* Choose the kernel variant and, for the blocked kernel, the number of fused time steps (1..4; 0 = default). */
+int rfa_configure(rfa_sim *s, int kernel, int fused_steps);
+
+/* Introspection: fused steps in use, kernel in use, number of kernel launches issued so far by this simulation. */
+int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launches);
+
+/* Host-only view of the blocked kernel's launch plan for a grid (no GPU needed; used by the unit tests
+ * and the bench report).  resident_ctas = CTAs that can be co-resident (SM count x occupancy).
+ * out = { ok, tiles_x, tiles_y, z_chunks, planes_per_chunk, work_items, ctas_launched }. */
+int rfa_plan_query(const int dims[3], int batch, int fused_steps, int resident_ctas, int out[7]);
+
+int rfa_synchronize(rfa_sim *s);
+void rfa_destroy(rfa_sim *s);
+const char *rfa_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RFA_H */

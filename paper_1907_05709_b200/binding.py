@@ -1,0 +1,234 @@
+"""Thin ctypes binding over the C ABI of librfa.so (include/rfa.h): argument marshalling only.
+
+PyTorch is used for exactly two things: the device workspace (a uint8 CUDA tensor handed to
+``rfa_create``) and the CUDA stream.  Every step of the hot path runs in the library's kernels; there
+is no Python / PyTorch / CPU fallback -- if librfa.so is missing, loading raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librfa.so")
+
+RFA_OK, RFA_E_INVALID, RFA_E_UNSTABLE, RFA_E_CUDA, RFA_E_NOMEM = 0, -1, -2, -3, -4
+SRC_OFF, SRC_DIRICHLET, SRC_POWER = 0, 1, 2
+KERNEL_AUTO, KERNEL_PLAIN, KERNEL_BLOCKED = 0, 1, 2
+TISSUE_HELD = 1
+MAX_TISSUES = 32
+
+# every symbol include/rfa.h declares
+EXPORTS = [
+    "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
+    "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
+    "rfa_query", "rfa_plan_query", "rfa_synchronize", "rfa_destroy", "rfa_last_error",
+]
+
+
+class RfaTissue(ctypes.Structure):
+    _fields_ = [("k", ctypes.c_float), ("rho", ctypes.c_float), ("cp", ctypes.c_float),
+                ("wb_cb", ctypes.c_float), ("q_m", ctypes.c_float), ("t_init", ctypes.c_float),
+                ("flags", ctypes.c_uint32)]
+
+
+class RfaError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"librfa error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen librfa.so and declare the prototypes.  Raises if the library has not been built
+    (``python -m paper_1907_05709_b200.build`` or ``__graft_entry__.build()``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build the CUDA library first "
+                           "(python paper_1907_05709_b200/build.py). There is no CPU fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    i3 = ctypes.POINTER(ctypes.c_int)
+    f3 = ctypes.POINTER(ctypes.c_float)
+    vp = ctypes.c_void_p
+    lib.rfa_workspace_bytes.argtypes = [i3, ctypes.c_int]
+    lib.rfa_workspace_bytes.restype = ctypes.c_size_t
+    lib.rfa_stability_number.argtypes = [f3, ctypes.POINTER(RfaTissue), ctypes.c_int, ctypes.c_float]
+    lib.rfa_stability_number.restype = ctypes.c_double
+    lib.rfa_create.argtypes = [ctypes.POINTER(vp), i3, f3, vp, ctypes.POINTER(RfaTissue), ctypes.c_int,
+                               ctypes.c_float, ctypes.c_float, ctypes.c_int, vp, ctypes.c_size_t, vp]
+    lib.rfa_create.restype = ctypes.c_int
+    lib.rfa_set_needle.argtypes = [vp, ctypes.c_int, f3, f3, vp, ctypes.c_int, ctypes.c_float]
+    lib.rfa_set_needle.restype = ctypes.c_int
+    lib.rfa_set_temperature.argtypes = [vp, ctypes.c_int, vp]
+    lib.rfa_set_temperature.restype = ctypes.c_int
+    lib.rfa_step.argtypes = [vp, ctypes.c_int]
+    lib.rfa_step.restype = ctypes.c_int
+    lib.rfa_get_temperature.argtypes = [vp, ctypes.c_int, vp]
+    lib.rfa_get_temperature.restype = ctypes.c_int
+    lib.rfa_get_necrosis.argtypes = [vp, ctypes.c_int, vp]
+    lib.rfa_get_necrosis.restype = ctypes.c_int
+    lib.rfa_necrotic_voxels.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
+    lib.rfa_necrotic_voxels.restype = ctypes.c_int
+    lib.rfa_configure.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+    lib.rfa_configure.restype = ctypes.c_int
+    lib.rfa_query.argtypes = [vp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int64)]
+    lib.rfa_query.restype = ctypes.c_int
+    lib.rfa_plan_query.argtypes = [i3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
+    lib.rfa_plan_query.restype = ctypes.c_int
+    lib.rfa_synchronize.argtypes = [vp]
+    lib.rfa_synchronize.restype = ctypes.c_int
+    lib.rfa_destroy.argtypes = [vp]
+    lib.rfa_destroy.restype = None
+    lib.rfa_last_error.argtypes = []
+    lib.rfa_last_error.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != RFA_OK:
+        raise RfaError(rc, load_library().rfa_last_error().decode("utf-8", "replace"))
+
+
+def tissue_array(table) -> ctypes.Array:
+    """numpy structured rows (k, rho, cp, wb_cb, q_m, t_init, flags) -> rfa_tissue[]"""
+    arr = (RfaTissue * len(table))()
+    for i, r in enumerate(table):
+        arr[i] = RfaTissue(float(r["k"]), float(r["rho"]), float(r["cp"]), float(r["wb_cb"]),
+                           float(r["q_m"]), float(r["t_init"]), int(r["flags"]))
+    return arr
+
+
+def _i3(v):
+    return (ctypes.c_int * 3)(*[int(x) for x in v])
+
+
+def _f3(v):
+    return (ctypes.c_float * 3)(*[float(x) for x in v])
+
+
+def stability_number(spacing_mm, table, dt) -> float:
+    lib = load_library()
+    return float(lib.rfa_stability_number(_f3(spacing_mm), tissue_array(table), len(table), float(dt)))
+
+
+def plan_query(dims, batch, fused, resident_ctas) -> dict:
+    lib = load_library()
+    out = (ctypes.c_int * 7)()
+    _check(lib.rfa_plan_query(_i3(dims), int(batch), int(fused), int(resident_ctas), out))
+    keys = ["ok", "tiles_x", "tiles_y", "z_chunks", "planes_per_chunk", "work_items", "ctas"]
+    return dict(zip(keys, [int(x) for x in out]))
+
+
+def _ptr(x):
+    """host numpy array or torch tensor (host or CUDA) -> raw address (the library tells them apart)"""
+    if isinstance(x, np.ndarray):
+        return ctypes.c_void_p(x.ctypes.data)
+    return ctypes.c_void_p(x.data_ptr())
+
+
+class RfaSim:
+    """One simulation: ``batch`` scenarios sharing a label volume.  Mirrors include/rfa.h one to one."""
+
+    def __init__(self, dims, spacing_mm, labels, table, t_blood: float, dt: float, batch: int = 1,
+                 device="cuda:0", stream=None):
+        import torch
+        self._torch = torch
+        lib = load_library()
+        self._lib = lib
+        self.dims = tuple(int(d) for d in dims)
+        self.batch = int(batch)
+        self.nvox = self.dims[0] * self.dims[1] * self.dims[2]
+        self.device = torch.device(device)
+        lab = np.ascontiguousarray(labels, dtype=np.uint8).reshape(-1)
+        if lab.size != self.nvox:
+            raise ValueError("labels do not match dims")
+        need = int(lib.rfa_workspace_bytes(_i3(dims), self.batch))
+        self._handle = ctypes.c_void_p()
+        with torch.cuda.device(self.device):
+            # PyTorch's only roles: device memory and the stream
+            self.workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=self.device)
+            st = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.stream = st
+            rc = lib.rfa_create(ctypes.byref(self._handle), _i3(dims), _f3(spacing_mm),
+                                ctypes.c_void_p(lab.ctypes.data), tissue_array(table), len(table),
+                                float(t_blood), float(dt), self.batch,
+                                ctypes.c_void_p(self.workspace.data_ptr()), need, ctypes.c_void_p(st.cuda_stream))
+        _check(rc)
+
+    # -- lifetime ----------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_handle", None) is not None and self._handle.value:
+            self._lib.rfa_destroy(self._handle)
+            self._handle = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the ABI, same names -------------------------------------------------------------------
+    def set_needle(self, scenario: int, mask, mode: int, value: float, tip_mm=None, axis=None):
+        m = None
+        if mode != SRC_OFF:
+            m = mask if not isinstance(mask, np.ndarray) else np.ascontiguousarray(mask, dtype=np.uint8)
+        _check(self._lib.rfa_set_needle(self._handle, int(scenario),
+                                        _f3(tip_mm) if tip_mm is not None else None,
+                                        _f3(axis) if axis is not None else None,
+                                        _ptr(m) if m is not None else None, int(mode), float(value)))
+
+    def set_temperature(self, scenario: int, t_c):
+        t = t_c if not isinstance(t_c, np.ndarray) else np.ascontiguousarray(t_c, dtype=np.float32)
+        _check(self._lib.rfa_set_temperature(self._handle, int(scenario), _ptr(t)))
+
+    def step(self, n: int = 1):
+        _check(self._lib.rfa_step(self._handle, int(n)))
+
+    def get_temperature(self, scenario: int = 0, out=None):
+        nx, ny, nz = self.dims
+        if out is None:
+            out = np.empty((nz, ny, nx), dtype=np.float32)
+        _check(self._lib.rfa_get_temperature(self._handle, int(scenario), _ptr(out)))
+        return out
+
+    def get_necrosis(self, scenario: int = 0, out=None):
+        nx, ny, nz = self.dims
+        if out is None:
+            out = np.empty((nz, ny, nx), dtype=np.uint8)
+        _check(self._lib.rfa_get_necrosis(self._handle, int(scenario), _ptr(out)))
+        return out
+
+    def necrotic_voxels(self, scenario: int = 0):
+        a, t = ctypes.c_int64(), ctypes.c_int64()
+        _check(self._lib.rfa_necrotic_voxels(self._handle, int(scenario), ctypes.byref(a), ctypes.byref(t)))
+        return int(a.value), int(t.value)
+
+    def configure(self, kernel: int = KERNEL_AUTO, fused_steps: int = 0):
+        _check(self._lib.rfa_configure(self._handle, int(kernel), int(fused_steps)))
+
+    def query(self) -> dict:
+        k, f, n = ctypes.c_int(), ctypes.c_int(), ctypes.c_int64()
+        _check(self._lib.rfa_query(self._handle, ctypes.byref(k), ctypes.byref(f), ctypes.byref(n)))
+        return {"kernel": int(k.value), "fused_steps": int(f.value), "kernel_launches": int(n.value)}
+
+    def synchronize(self):
+        _check(self._lib.rfa_synchronize(self._handle))
+
+
+def from_workload(w, device="cuda:0", stream=None) -> RfaSim:
+    """Convenience: create a simulation from a ``workloads.Workload`` and place its needles."""
+    sim = RfaSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt, batch=w.batch,
+                 device=device, stream=stream)
+    if w.t0 is not None:
+        for b in range(w.batch):
+            sim.set_temperature(b, np.asarray(w.t0, dtype=np.float32))
+    for b, nd in enumerate(w.needles):
+        sim.set_needle(b, nd.mask, nd.mode, nd.value, nd.tip_mm, nd.axis)
+    return sim

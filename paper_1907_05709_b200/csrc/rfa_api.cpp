@@ -1,0 +1,539 @@
+// rfa_api.cpp -- host logic and the C ABI of librfa.so (include/rfa.h).
+//
+// Host side of the hot path: validation, the per-label coefficient table in fp64 (rounded once to
+// fp32), the monotone stability check, workspace layout, the plan of the temporally blocked kernel,
+// ping-pong bookkeeping (Alg. 2).  All device work goes through the launchers of
+// rfa_kernels.cu on the caller's stream.  There is no CPU fallback: without a CUDA device rfa_create
+// fails with RFA_E_CUDA.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/rfa.h"
+#include "rfa_internal.h"
+
+static thread_local std::string g_err;
+
+static int fail(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+static int cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(RFA_E_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+struct rfa_sim {
+    RfaGrid g{};
+    size_t nvox = 0;
+    double h_m[3]{};                     // spacing in metres
+    double dt = 0, t_blood = 0;
+    std::vector<rfa_tissue> table;
+    uint32_t label_held_mask = 0;
+    std::vector<double> q_power;         // per scenario, W/m^3 (0 unless a POWER needle is set)
+    cudaStream_t stream = nullptr;
+    unsigned char *ws = nullptr;         // device workspace
+    bool own_ws = false;
+    float *theta[2]{};                   // ping-pong temperature images (theta = T - T_a)
+    int cur = 0;                         // index of the current image
+    uint8_t *state = nullptr;            // packed state bytes
+    float *tables = nullptr;             // batch x 3 x 128 coefficients
+    unsigned char *scratch = nullptr;    // nvox*4 bytes staging
+    unsigned long long *counters = nullptr;
+    int kernel = RFA_KERNEL_AUTO;
+    int fused = 2;
+    RfaTbPlan plans[5]{};                // index = fused steps 1..4
+    int resident[5]{};
+    long long launches = 0;
+};
+
+// ------------------------------------------------------------------------------------------------
+// workspace layout
+// ------------------------------------------------------------------------------------------------
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct WsLayout {
+    size_t theta0, theta1, state, tables, scratch, counters, total;
+};
+
+static bool ws_layout(const int dims[3], int batch, WsLayout &L)
+{
+    if (!dims || batch < 1) return false;
+    for (int a = 0; a < 3; ++a)
+        if (dims[a] < 1) return false;
+    const double nv = (double)dims[0] * dims[1] * dims[2];
+    if (nv * batch > 1.0e11) return false;
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    size_t off = 0;
+    L.theta0 = off;
+    off = align256(off + nvox * batch * 4);
+    L.theta1 = off;
+    off = align256(off + nvox * batch * 4);
+    L.state = off;
+    off = align256(off + nvox * batch);
+    L.tables = off;
+    off = align256(off + (size_t)batch * 3 * RFA_TABLE_N * 4);
+    L.scratch = off;
+    off = align256(off + nvox * 4);
+    L.counters = off;
+    off = align256(off + 256);
+    L.total = off;
+    return true;
+}
+
+extern "C" size_t rfa_workspace_bytes(const int dims[3], int batch)
+{
+    WsLayout L;
+    return ws_layout(dims, batch, L) ? L.total : 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// host numerics
+// ------------------------------------------------------------------------------------------------
+static bool tissue_ok(const rfa_tissue &t)
+{
+    if (!std::isfinite(t.k) || !std::isfinite(t.rho) || !std::isfinite(t.cp) || !std::isfinite(t.wb_cb) ||
+        !std::isfinite(t.q_m) || !std::isfinite(t.t_init))
+        return false;
+    if (t.flags & RFA_TISSUE_HELD) return true;
+    return t.k > 0.f && t.rho > 0.f && t.cp > 0.f && t.wb_cb >= 0.f;
+}
+
+extern "C" double rfa_stability_number(const float spacing_mm[3], const rfa_tissue *table, int n_tissue, float dt_s)
+{
+    if (!spacing_mm || !table || n_tissue < 1 || !(dt_s > 0.f)) return -1.0;
+    double w = 0;
+    for (int a = 0; a < 3; ++a) {
+        if (!(spacing_mm[a] > 0.f) || !std::isfinite(spacing_mm[a])) return -1.0;
+        const double h = (double)spacing_mm[a] * 1.0e-3;
+        w += 1.0 / (h * h);
+    }
+    double worst = 0;
+    for (int l = 0; l < n_tissue; ++l) {
+        const rfa_tissue &t = table[l];
+        if (!tissue_ok(t)) return -1.0;
+        if (t.flags & RFA_TISSUE_HELD) continue;
+        const double rc = (double)t.rho * t.cp;
+        worst = std::max(worst, (double)dt_s * (2.0 * (double)t.k / rc * w + (double)t.wb_cb / rc));
+    }
+    return worst;
+}
+
+// coefficient table of one scenario (see rfa_device.cuh); fp64, rounded once
+static void build_table(const rfa_sim *s, double q_power, RfaTableHost &out)
+{
+    const double W = 1.0 / (s->h_m[0] * s->h_m[0]) + 1.0 / (s->h_m[1] * s->h_m[1]) + 1.0 / (s->h_m[2] * s->h_m[2]);
+    for (int e = 0; e < RFA_TABLE_N; ++e) {
+        const int l = e & (int)RFA_ST_LABEL;
+        const bool dir = (e & (int)RFA_ST_DIRICHLET) != 0;
+        const bool pow = (e & (int)RFA_ST_POWER) != 0;
+        double a = 0, nk = 0, qa = 0;
+        if (l < (int)s->table.size() && !dir && !(s->table[l].flags & RFA_TISSUE_HELD)) {
+            const rfa_tissue &t = s->table[l];
+            const double kw = (double)t.k * W;
+            a = s->dt / ((double)t.rho * t.cp) * kw;
+            nk = -(2.0 + (double)t.wb_cb / kw);
+            qa = ((double)t.q_m + (pow ? q_power : 0.0)) / kw;
+        }
+        out.a[e] = (float)a;
+        out.nk[e] = (float)nk;
+        out.qa[e] = (float)qa;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// plan of the blocked kernel (host only)
+// ------------------------------------------------------------------------------------------------
+RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int resident_ctas)
+{
+    RfaTbPlan p{};
+    p.fused = fused;
+    const int S = fused;
+    if (S < 1 || S > 4 || nx < 4 || (nx % 4) != 0 || ny < S || nz < S || batch < 1 || resident_ctas < 1) return p;
+    const int BX = RFA_TB_BX, BY = RFA_TB_BY;
+    p.tiles_x = nx <= BX ? 1 : (nx - 8 + (BX - 8) - 1) / (BX - 8);
+    p.tiles_y = (ny + (BY - 2 * S) - 1) / (BY - 2 * S);
+    const long long per_z = (long long)p.tiles_x * p.tiles_y * batch;
+    // choose the number of z chunks: minimise rounds * (planes streamed per item + fixed cost)
+    double best = 1e300;
+    for (int nzc = 1; nzc <= nz; ++nzc) {
+        const int zchunk = (nz + nzc - 1) / nzc;
+        if ((nzc - 1) * zchunk >= nz) continue;              // empty last chunk
+        const long long items = per_z * nzc;
+        const long long rounds = (items + resident_ctas - 1) / resident_ctas;
+        const double cost = (double)rounds * (zchunk + 2 * S + 3);
+        if (cost < best - 1e-9) {
+            best = cost;
+            p.nzc = nzc;
+            p.zchunk = zchunk;
+        }
+    }
+    const long long items = per_z * p.nzc;
+    if (items > 0x7fffffffLL) return p;
+    p.n_items = (int)items;
+    p.grid = (int)std::min<long long>(items, resident_ctas);
+    p.ok = 1;
+    return p;
+}
+
+// exported for the CPU unit tests of the planner (no GPU needed)
+extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resident_ctas, int out[7])
+{
+    if (!dims || !out) return RFA_E_INVALID;
+    RfaTbPlan p = rfa_plan_blocked(dims[0], dims[1], dims[2], batch, fused, resident_ctas);
+    out[0] = p.ok;
+    out[1] = p.tiles_x;
+    out[2] = p.tiles_y;
+    out[3] = p.nzc;
+    out[4] = p.zchunk;
+    out[5] = p.n_items;
+    out[6] = p.grid;
+    return RFA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// helpers
+// ------------------------------------------------------------------------------------------------
+static bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes at{};
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static int check_sim(rfa_sim *s, int scenario)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (scenario < 0 || scenario >= s->g.batch) return fail(RFA_E_INVALID, "scenario %d out of range [0,%d)", scenario, s->g.batch);
+    return RFA_OK;
+}
+
+static int upload_table(rfa_sim *s, int scenario)
+{
+    RfaTableHost t;
+    build_table(s, s->q_power[scenario], t);
+    cudaError_t e = rfa_launch_table(t, s->tables + (size_t)scenario * 3 * RFA_TABLE_N, s->stream);
+    s->launches++;
+    if (e != cudaSuccess) return cuda_fail(e, "table upload");
+    return RFA_OK;
+}
+
+static void make_plans(rfa_sim *s)
+{
+    for (int f = 1; f <= 4; ++f) {
+        s->resident[f] = rfa_blocked_resident_ctas(f);
+        s->plans[f] = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, s->resident[f]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------------
+extern "C" const char *rfa_last_error(void) { return g_err.c_str(); }
+
+extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_mm[3], const uint8_t *labels,
+                          const rfa_tissue *table, int n_tissue, float t_blood_c, float dt_s, int batch,
+                          void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return fail(RFA_E_INVALID, "out is null");
+    *out = nullptr;
+    if (!dims || !spacing_mm || !labels || !table) return fail(RFA_E_INVALID, "null argument");
+    if (n_tissue < 1 || n_tissue > RFA_MAX_TISSUES) return fail(RFA_E_INVALID, "n_tissue %d outside 1..%d", n_tissue, RFA_MAX_TISSUES);
+    if (batch < 1) return fail(RFA_E_INVALID, "batch must be >= 1");
+    if (!(dt_s > 0.f) || !std::isfinite(dt_s)) return fail(RFA_E_INVALID, "dt must be positive and finite");
+    if (!std::isfinite(t_blood_c)) return fail(RFA_E_INVALID, "t_blood must be finite");
+    WsLayout L;
+    if (!ws_layout(dims, batch, L)) return fail(RFA_E_INVALID, "dims must be positive (and the volume of sane size)");
+    for (int a = 0; a < 3; ++a)
+        if (!(spacing_mm[a] > 0.f) || !std::isfinite(spacing_mm[a])) return fail(RFA_E_INVALID, "spacing must be positive and finite");
+    for (int l = 0; l < n_tissue; ++l)
+        if (!tissue_ok(table[l])) return fail(RFA_E_INVALID, "tissue row %d: non-finite or non-positive constants", l);
+    const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    {
+        unsigned mx = 0;
+        for (size_t v = 0; v < nvox; ++v) mx = std::max<unsigned>(mx, labels[v]);
+        if ((int)mx >= n_tissue) return fail(RFA_E_INVALID, "label id %u >= n_tissue %d", mx, n_tissue);
+    }
+    const double stab = rfa_stability_number(spacing_mm, table, n_tissue, dt_s);
+    if (stab < 0) return fail(RFA_E_INVALID, "invalid constants");
+    if (stab > 1.0)
+        return fail(RFA_E_UNSTABLE, "dt = %g s violates the monotone bound: dt*(2 alpha sum 1/h^2 + beta/(rho cp)) = %.4f > 1", (double)dt_s, stab);
+    if (workspace) {
+        if (workspace_bytes < L.total) return fail(RFA_E_INVALID, "workspace of %zu bytes < required %zu", workspace_bytes, L.total);
+        if (((uintptr_t)workspace & 255) != 0) return fail(RFA_E_INVALID, "workspace must be 256-byte aligned");
+    }
+
+    rfa_sim *s = new (std::nothrow) rfa_sim;
+    if (!s) return fail(RFA_E_NOMEM, "host allocation failed");
+    s->g.nx = dims[0];
+    s->g.ny = dims[1];
+    s->g.nz = dims[2];
+    s->g.batch = batch;
+    s->nvox = nvox;
+    double W = 0;
+    for (int a = 0; a < 3; ++a) {
+        s->h_m[a] = (double)spacing_mm[a] * 1.0e-3;          // mm -> m (PAPER.md:115 vs :104)
+        W += 1.0 / (s->h_m[a] * s->h_m[a]);
+    }
+    s->g.wx = (float)(1.0 / (s->h_m[0] * s->h_m[0]) / W);
+    s->g.wy = (float)(1.0 / (s->h_m[1] * s->h_m[1]) / W);
+    s->g.wz = (float)(1.0 / (s->h_m[2] * s->h_m[2]) / W);
+    s->dt = dt_s;
+    s->t_blood = t_blood_c;
+    s->g.t_blood = t_blood_c;
+    s->g.thr = (float)(60.0 - (double)t_blood_c);            // T >= 60 C  (R-11)
+    s->table.assign(table, table + n_tissue);
+    for (int l = 0; l < n_tissue; ++l)
+        if (table[l].flags & RFA_TISSUE_HELD) s->label_held_mask |= 1u << l;
+    s->q_power.assign(batch, 0.0);
+    s->stream = (cudaStream_t)cuda_stream;
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) {
+        delete s;
+        cudaGetLastError();
+        return fail(RFA_E_CUDA, "no CUDA device (%s); librfa has no CPU fallback", e != cudaSuccess ? cudaGetErrorString(e) : "count = 0");
+    }
+    if (workspace) {
+        if (!is_device_ptr(workspace)) {
+            delete s;
+            return fail(RFA_E_INVALID, "workspace is not device memory");
+        }
+        s->ws = (unsigned char *)workspace;
+    } else {
+        e = cudaMalloc((void **)&s->ws, L.total);
+        if (e != cudaSuccess) {
+            delete s;
+            cudaGetLastError();
+            return fail(RFA_E_NOMEM, "cudaMalloc of %zu bytes failed: %s", L.total, cudaGetErrorString(e));
+        }
+        s->own_ws = true;
+    }
+    s->theta[0] = (float *)(s->ws + L.theta0);
+    s->theta[1] = (float *)(s->ws + L.theta1);
+    s->state = s->ws + L.state;
+    s->tables = (float *)(s->ws + L.tables);
+    s->scratch = s->ws + L.scratch;
+    s->counters = (unsigned long long *)(s->ws + L.counters);
+
+    int rc = RFA_OK;
+    do {
+        // labels -> device (staged through scratch), then label -> initial temperature image
+        e = cudaMemcpyAsync(s->scratch, labels, nvox, cudaMemcpyHostToDevice, s->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "label upload"); break; }
+        float theta0[32];
+        for (int l = 0; l < 32; ++l) theta0[l] = l < n_tissue ? (float)((double)table[l].t_init - (double)t_blood_c) : 0.f;
+        e = rfa_launch_init(s->g, s->scratch, theta0, s->theta[0], s->state, s->stream);
+        s->launches++;
+        if (e != cudaSuccess) { rc = cuda_fail(e, "init kernel"); break; }
+        for (int b = 0; b < batch && rc == RFA_OK; ++b) rc = upload_table(s, b);
+        if (rc != RFA_OK) break;
+        make_plans(s);
+        e = cudaStreamSynchronize(s->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "create"); break; }
+    } while (0);
+    if (rc != RFA_OK) {
+        if (s->own_ws) cudaFree(s->ws);
+        delete s;
+        return rc;
+    }
+    *out = s;
+    return RFA_OK;
+}
+
+extern "C" void rfa_destroy(rfa_sim *s)
+{
+    if (!s) return;
+    cudaStreamSynchronize(s->stream);
+    if (s->own_ws) cudaFree(s->ws);
+    delete s;
+}
+
+extern "C" int rfa_set_needle(rfa_sim *s, int scenario, const float tip_mm[3], const float axis[3],
+                              const uint8_t *mask, int mode, float value)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    if (mode != RFA_SRC_OFF && mode != RFA_SRC_DIRICHLET && mode != RFA_SRC_POWER) return fail(RFA_E_INVALID, "bad source mode %d", mode);
+    if (mode != RFA_SRC_OFF && !mask) return fail(RFA_E_INVALID, "mask is null");
+    if (mode != RFA_SRC_OFF && !std::isfinite(value)) return fail(RFA_E_INVALID, "source value must be finite");
+    for (int a = 0; a < 3; ++a) {
+        if (tip_mm && !std::isfinite(tip_mm[a])) return fail(RFA_E_INVALID, "tip position must be finite");
+        if (axis && !std::isfinite(axis[a])) return fail(RFA_E_INVALID, "axis must be finite");
+    }
+    const uint8_t *mdev = nullptr;
+    cudaError_t e;
+    if (mode != RFA_SRC_OFF) {
+        if (is_device_ptr(mask)) {
+            mdev = mask;
+        } else {
+            e = cudaMemcpyAsync(s->scratch, mask, s->nvox, cudaMemcpyHostToDevice, s->stream);
+            if (e != cudaSuccess) return cuda_fail(e, "mask upload");
+            mdev = s->scratch;
+        }
+    }
+    const float theta_value = (float)((double)value - s->t_blood);
+    e = rfa_launch_needle(s->g, scenario, mdev, mode, theta_value, s->theta[s->cur], s->state, s->stream);
+    s->launches++;
+    if (e != cudaSuccess) return cuda_fail(e, "needle kernel");
+    s->q_power[scenario] = (mode == RFA_SRC_POWER) ? (double)value : 0.0;
+    rc = upload_table(s, scenario);
+    if (rc) return rc;
+    if (mdev == s->scratch) {                               // the host mask may be reused by the caller
+        e = cudaStreamSynchronize(s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "set_needle");
+    }
+    return RFA_OK;
+}
+
+extern "C" int rfa_set_temperature(rfa_sim *s, int scenario, const float *t_c)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    if (!t_c) return fail(RFA_E_INVALID, "t_c is null");
+    const float *src = t_c;
+    cudaError_t e;
+    const bool dev = is_device_ptr(t_c);
+    if (!dev) {
+        e = cudaMemcpyAsync(s->scratch, t_c, s->nvox * 4, cudaMemcpyHostToDevice, s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "temperature upload");
+        src = (const float *)s->scratch;
+    }
+    e = rfa_launch_set_temperature(s->g, scenario, src, s->theta[s->cur], s->state, s->stream);
+    s->launches++;
+    if (e != cudaSuccess) return cuda_fail(e, "set_temperature kernel");
+    if (!dev) {
+        e = cudaStreamSynchronize(s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "set_temperature");
+    }
+    return RFA_OK;
+}
+
+extern "C" int rfa_configure(rfa_sim *s, int kernel, int fused_steps)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (kernel != RFA_KERNEL_AUTO && kernel != RFA_KERNEL_PLAIN && kernel != RFA_KERNEL_BLOCKED) return fail(RFA_E_INVALID, "bad kernel id %d", kernel);
+    if (fused_steps < 0 || fused_steps > 4) return fail(RFA_E_INVALID, "fused_steps must be 0..4");
+    const int f = fused_steps == 0 ? 2 : fused_steps;
+    if (kernel == RFA_KERNEL_BLOCKED && !s->plans[f].ok)
+        return fail(RFA_E_INVALID, "the blocked kernel needs nx %% 4 == 0 and ny, nz >= fused steps (grid %dx%dx%d, fused %d)", s->g.nx, s->g.ny, s->g.nz, f);
+    s->kernel = kernel;
+    s->fused = f;
+    return RFA_OK;
+}
+
+extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launches)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
+    if (kernel) *kernel = blocked ? RFA_KERNEL_BLOCKED : RFA_KERNEL_PLAIN;
+    if (fused_steps) *fused_steps = blocked ? s->fused : 1;
+    if (kernel_launches) *kernel_launches = s->launches;
+    return RFA_OK;
+}
+
+extern "C" int rfa_step(rfa_sim *s, int n)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (n < 0) return fail(RFA_E_INVALID, "n must be >= 0");
+    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
+    while (n > 0) {
+        cudaError_t e;
+        int did = 1;
+        if (blocked) {
+            did = std::min(n, s->fused);
+            while (did > 1 && !s->plans[did].ok) --did;
+            if (s->plans[did].ok)
+                e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->state, s->tables, s->stream);
+            else
+                e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->state, s->tables, s->stream);
+        } else {
+            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->state, s->tables, s->stream);
+        }
+        s->launches++;
+        if (e != cudaSuccess) return cuda_fail(e, "step kernel");
+        s->cur ^= 1;                                        // Alg. 2: swap the two buffers
+        n -= did;
+    }
+    return RFA_OK;
+}
+
+extern "C" int rfa_synchronize(rfa_sim *s)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    cudaError_t e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "synchronize");
+    return RFA_OK;
+}
+
+extern "C" int rfa_get_temperature(rfa_sim *s, int scenario, float *out)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    if (!out) return fail(RFA_E_INVALID, "out is null");
+    const bool dev = is_device_ptr(out);
+    float *dst = dev ? out : (float *)s->scratch;
+    cudaError_t e = rfa_launch_get_temperature(s->g, scenario, s->theta[s->cur], dst, s->stream);
+    s->launches++;
+    if (e != cudaSuccess) return cuda_fail(e, "get_temperature kernel");
+    if (!dev) {
+        e = cudaMemcpyAsync(out, dst, s->nvox * 4, cudaMemcpyDeviceToHost, s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "temperature download");
+    }
+    e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "get_temperature");
+    return RFA_OK;
+}
+
+extern "C" int rfa_get_necrosis(rfa_sim *s, int scenario, uint8_t *out)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    if (!out) return fail(RFA_E_INVALID, "out is null");
+    const bool dev = is_device_ptr(out);
+    uint8_t *dst = dev ? out : s->scratch;
+    cudaError_t e = rfa_launch_get_necrosis(s->g, scenario, s->state, dst, s->stream);
+    s->launches++;
+    if (e != cudaSuccess) return cuda_fail(e, "get_necrosis kernel");
+    if (!dev) {
+        e = cudaMemcpyAsync(out, dst, s->nvox, cudaMemcpyDeviceToHost, s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "necrosis download");
+    }
+    e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "get_necrosis");
+    return RFA_OK;
+}
+
+extern "C" int rfa_necrotic_voxels(rfa_sim *s, int scenario, int64_t *all_voxels, int64_t *tissue_voxels)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    cudaError_t e = rfa_launch_count(s->g, scenario, s->state, s->label_held_mask, s->counters, s->stream);
+    s->launches++;
+    if (e != cudaSuccess) return cuda_fail(e, "count kernel");
+    unsigned long long h[2] = {0, 0};
+    e = cudaMemcpyAsync(h, s->counters, sizeof h, cudaMemcpyDeviceToHost, s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "count download");
+    e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "necrotic_voxels");
+    if (all_voxels) *all_voxels = (int64_t)h[0];
+    if (tissue_voxels) *tissue_voxels = (int64_t)h[1];
+    return RFA_OK;
+}

@@ -1,0 +1,54 @@
+// rfa_device.cuh -- the one per-voxel arithmetic every kernel of librfa.so shares, and the packed
+// per-voxel state byte.  (Product code; the fp64 oracle under oracle/ shares nothing with this.)
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+// ---- packed state byte (one per voxel per scenario) ---------------------------------------------
+//   bits 0..4  label id (<= 32 tissues, "voxel-wise" parameters)
+//   bit  5     needle voxel, Dirichlet: held at its temperature (Alg. 1 :306)
+//   bit  6     needle voxel, constant power source (R-17)
+//   bit  7     necrotic: T reached 60 C at some step (sticky)
+// bits 0..6 index the per-scenario coefficient table (128 entries).
+#define RFA_ST_LABEL 0x1fu
+#define RFA_ST_DIRICHLET 0x20u
+#define RFA_ST_POWER 0x40u
+#define RFA_ST_NECRO 0x80u
+#define RFA_ST_INDEX 0x7fu
+#define RFA_TABLE_N 128
+
+// Per-scenario coefficient table, three planes of RFA_TABLE_N floats each (fp64 on the host,
+// rounded once):
+//   a[e]   = dt K /(rho c_p) * W          W = 1/dx^2 + 1/dy^2 + 1/dz^2 (metres)      (0 for held entries)
+//   nk[e]  = -(2 + w_b c_b /(K W))        (0 for held entries)
+//   qa[e]  = (Q_m + Q_power) / (K W)      (0 for held entries)
+// and three global weights wx = (1/dx^2)/W, wy, wz.
+struct RfaTableHost {
+    float a[RFA_TABLE_N];
+    float nk[RFA_TABLE_N];
+    float qa[RFA_TABLE_N];
+};
+
+// theta' for one voxel.  theta = T - T_a.  Eq. 12 rearranged as
+//   theta' = theta + a * ( wx (xm+xp) + wy (ym+yp) + wz (zm+zp) + qa - (2 + p/a) theta )
+// Explicit intrinsics fix the rounding sequence, so every kernel variant is bit-identical.
+// A held voxel has a = 0 and returns theta exactly (Eq. 13, Alg. 1 :313).
+__device__ __forceinline__ float rfa_update(float t, float xm, float xp, float ym, float yp, float zm,
+                                            float zp, float a, float nk, float qa, float wx, float wy,
+                                            float wz)
+{
+    const float sx = __fadd_rn(xm, xp);
+    const float sy = __fadd_rn(ym, yp);
+    const float sz = __fadd_rn(zm, zp);
+    const float l = __fmaf_rn(wz, sz, __fmaf_rn(wy, sy, __fmaf_rn(wx, sx, qa)));
+    const float g = __fmaf_rn(nk, t, l);
+    return __fmaf_rn(a, g, t);
+}
+
+__device__ __forceinline__ int rfa_reflect(int j, int n)
+{
+    // mirror about the outer faces (ghost -1 -> 0, -2 -> 1, n -> n-1 ...), then clamp
+    if (j < 0) j = -1 - j;
+    if (j >= n) j = 2 * n - 1 - j;
+    return min(max(j, 0), n - 1);
+}

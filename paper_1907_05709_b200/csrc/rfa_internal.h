@@ -1,0 +1,52 @@
+// rfa_internal.h -- host-side declarations shared by rfa_api.cpp (host logic, C ABI) and
+// rfa_kernels.cu (sm_100a kernels + launchers).  Not part of the public boundary.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "rfa_device.cuh"
+
+struct RfaGrid {
+    int nx, ny, nz, batch;
+    float wx, wy, wz;   // normalised 1/h^2 weights (sum = 1)
+    float thr;          // necrosis threshold in theta = T - T_a
+    float t_blood;
+};
+
+// Plan of the temporally blocked kernel for one launch geometry.
+struct RfaTbPlan {
+    int fused;                 // S: time steps per launch, 1..4
+    int tiles_x, tiles_y;      // xy tiling
+    int nzc, zchunk;           // z chunks
+    int n_items;               // batch * nzc * tiles_y * tiles_x
+    int grid;                  // CTAs launched (persistent, static round-robin over items)
+    int ok;                    // 0: this grid cannot use the blocked kernel
+};
+
+// tile constants of the blocked kernel (one configuration in round 1)
+enum { RFA_TB_TX = 16, RFA_TB_TY = 16, RFA_TB_RY = 4, RFA_TB_BX = 4 * RFA_TB_TX, RFA_TB_BY = RFA_TB_RY * RFA_TB_TY };
+
+// host-only planning (no CUDA calls): implemented in rfa_api.cpp, unit-tested on CPU
+RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int resident_ctas);
+
+// launchers (rfa_kernels.cu).  All asynchronous on `st`; return cudaGetLastError().
+cudaError_t rfa_launch_table(const RfaTableHost &tbl, float *dst, cudaStream_t st);
+cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const float *theta0_by_label /*dev, 32*/,
+                            float *theta, uint8_t *state, cudaStream_t st);
+cudaError_t rfa_launch_needle(const RfaGrid &g, int scenario, const uint8_t *mask_dev /*may be null*/, int mode,
+                              float theta_value, float *theta, uint8_t *state, cudaStream_t st);
+cudaError_t rfa_launch_set_temperature(const RfaGrid &g, int scenario, const float *t_dev, float *theta,
+                                       uint8_t *state, cudaStream_t st);
+cudaError_t rfa_launch_get_temperature(const RfaGrid &g, int scenario, const float *theta, float *out_dev,
+                                       cudaStream_t st);
+cudaError_t rfa_launch_get_necrosis(const RfaGrid &g, int scenario, const uint8_t *state, uint8_t *out_dev,
+                                    cudaStream_t st);
+cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *state, uint32_t label_held_mask,
+                             unsigned long long *counters_dev /*2*/, cudaStream_t st);
+cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, uint8_t *state, const float *tables,
+                             cudaStream_t st);
+cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
+                               uint8_t *state, const float *tables, cudaStream_t st);
+// resident CTAs of the blocked kernel on the current device for `fused` steps (occupancy * SM count)
+int rfa_blocked_resident_ctas(int fused);

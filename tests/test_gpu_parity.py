@@ -1,0 +1,308 @@
+"""GPU parity tests: the CUDA path (through the C ABI of librfa.so) against the fp64 oracle, element by
+element on the same seeded inputs.
+
+Bars (BASELINE.json north_star): max |dT| <= 1e-3 C after the configured number of steps; the necrosis
+mask identical except for voxels whose oracle temperature lies within 1e-3 C of 60 C (counted).  Kernel
+variants must agree bit for bit (integer/byte work and the shared fp32 arithmetic).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1907_05709_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1.0e-3        # deg C, north_star
+BAND = 1.0e-3       # exempt band around 60 C, north_star
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+@pytest.fixture(scope="module")
+def rfa():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_1907_05709_b200 import binding, build
+    build.build()
+    binding.load_library()          # raises if librfa.so is missing: no fallback
+    return binding
+
+
+def run_gpu(rfa, w, steps, kernel=None, fused=0, scenario_list=None):
+    sim = rfa.from_workload(w)
+    if kernel is not None:
+        sim.configure(kernel, fused)
+    sim.step(steps)
+    sc = range(w.batch) if scenario_list is None else scenario_list
+    T = [sim.get_temperature(b) for b in sc]
+    N = [sim.get_necrosis(b) for b in sc]
+    q = sim.query()
+    sim.close()
+    return T, N, q
+
+
+def compare(T_gpu, N_gpu, osim, tol=TOL):
+    To = osim.T
+    err = float(np.max(np.abs(T_gpu.astype(np.float64) - To)))
+    assert err <= tol, f"max |dT| = {err:.3e} > {tol}"
+    mism = (N_gpu != 0) != (osim.necro != 0)
+    exempt = np.abs(To - 60.0) <= BAND
+    bad = int((mism & ~exempt).sum())
+    assert bad == 0, f"{bad} necrosis mismatches outside the +-{BAND} C band ({int(mism.sum())} inside)"
+    return err, int((mism & exempt).sum())
+
+
+# ----------------------------------------------------------------------------------------------
+# small ragged cases: several tiles, ragged tails, all labels, both source modes
+# ----------------------------------------------------------------------------------------------
+RAGGED = [
+    dict(dims=(136, 70, 21), spacing=(0.7, 0.9, 1.3), steps=37, mode=W.SRC_DIRICHLET, value=90.0),
+    dict(dims=(72, 130, 19), spacing=(1.1, 0.8, 0.9), steps=41, mode=W.SRC_POWER, value=2.0e7),
+    dict(dims=(44, 38, 29), spacing=(1.0, 1.0, 1.0), steps=50, mode=W.SRC_DIRICHLET, value=60.0),
+    dict(dims=(45, 38, 29), spacing=(0.7, 0.9, 1.3), steps=30, mode=W.SRC_DIRICHLET, value=90.0),   # nx % 4 != 0
+]
+
+
+@pytest.mark.parametrize("case", RAGGED, ids=lambda c: "x".join(map(str, c["dims"])))
+def test_ragged_parity_and_variants(rfa, oracle, case):
+    w = W.ragged_phantom(dims=case["dims"], spacing=case["spacing"], steps=case["steps"], mode=case["mode"],
+                         value=case["value"], q_m=10714.0, dt=0.05)
+    w.table["t_init"][W.KIDNEY] = 36.0          # a label whose initial temperature differs from T_a
+    osim = oracle.run_workload(w)
+    Tp, Np, qp = run_gpu(rfa, w, w.steps, rfa.KERNEL_PLAIN)
+    assert qp["kernel"] == rfa.KERNEL_PLAIN
+    err, n_band = compare(Tp[0], Np[0], osim)
+    assert err < 2e-4                            # far inside the bar on short runs
+    if case["dims"][0] % 4 == 0:
+        for fused in (1, 2, 3, 4):
+            Tb, Nb, qb = run_gpu(rfa, w, w.steps, rfa.KERNEL_BLOCKED, fused)
+            assert qb["kernel"] == rfa.KERNEL_BLOCKED and qb["fused_steps"] == fused
+            assert np.array_equal(Tb[0].view(np.uint32), Tp[0].view(np.uint32)), f"fused={fused} differs from plain"
+            assert np.array_equal(Nb[0], Np[0])
+    else:
+        Ta, Na, qa = run_gpu(rfa, w, w.steps, rfa.KERNEL_AUTO)
+        assert qa["kernel"] == rfa.KERNEL_PLAIN     # falls back to the plain CUDA kernel, still on the GPU
+        assert np.array_equal(Ta[0], Tp[0])
+        with pytest.raises(rfa.RfaError):
+            rfa.from_workload(w).configure(rfa.KERNEL_BLOCKED, 2)
+
+
+def test_batched_scenarios(rfa, oracle):
+    w = W.ragged_phantom(dims=(68, 66, 23), spacing=(1.0, 1.0, 1.2), steps=33, batch=5, dt=0.08)
+    T, N, q = run_gpu(rfa, w, w.steps, rfa.KERNEL_BLOCKED, 2)
+    Tp, Np, _ = run_gpu(rfa, w, w.steps, rfa.KERNEL_PLAIN)
+    for b in range(w.batch):
+        osim = oracle.run_workload(w, scenario=b)
+        compare(T[b], N[b], osim)
+        assert np.array_equal(T[b], Tp[b]) and np.array_equal(N[b], Np[b])
+    assert not np.array_equal(T[0], T[1])       # the scenarios really differ
+
+
+def test_needle_semantics(rfa, oracle):
+    """Override (R-15), release (R-16), sticky necrosis (R-12), inclusive threshold (R-11), counts (R-13)."""
+    n = 12
+    lab = np.ones((n, n, n), np.uint8)
+    lab[4, 4, 5] = W.VESSEL
+    table = W.tissue_table()
+    m1 = np.zeros((n, n, n), np.uint8)
+    m1[4, 4, 4] = 1
+    m1[4, 4, 5] = 1
+    m2 = np.zeros((n, n, n), np.uint8)
+    m2[1, 1, 1] = 1
+    osim = oracle.OracleSim((n, n, n), (1.0, 1.0, 1.0), lab, table, 37.0, 0.1)
+    sim = rfa.RfaSim((n, n, n), (1.0, 1.0, 1.0), lab, table, 37.0, 0.1)
+    for s in (osim,):
+        s.set_needle(m1, W.SRC_DIRICHLET, 90.0)
+    sim.set_needle(0, m1, rfa.SRC_DIRICHLET, 90.0)
+    osim.step(200)
+    sim.step(200)
+    compare(sim.get_temperature(0), sim.get_necrosis(0), osim)
+    osim.set_needle(m2, W.SRC_DIRICHLET, 59.9995)
+    sim.set_needle(0, m2, rfa.SRC_DIRICHLET, 59.9995)
+    osim.step(1)
+    sim.step(1)
+    T = sim.get_temperature(0)
+    assert T[4, 4, 5] == 90.0 and T[4, 4, 4] < 90.0 and abs(T[1, 1, 1] - 59.9995) < 1e-5
+    osim.step(1500)
+    sim.step(1500)
+    compare(sim.get_temperature(0), sim.get_necrosis(0), osim)
+    N = sim.get_necrosis(0)
+    assert N[1, 1, 1] == 0 and N[4, 4, 4] == 1
+    all_v, tissue_v = sim.necrotic_voxels(0)
+    assert all_v == int(N.sum())
+    held_or_needle = ((table["flags"][lab] & 1) != 0) | (m2 != 0)
+    assert tissue_v == int((N != 0)[~held_or_needle].sum())
+    sim.set_needle(0, None, rfa.SRC_OFF, 0.0)
+    osim.set_needle(None, W.SRC_OFF, 0.0)
+    sim.step(3)
+    osim.step(3)
+    compare(sim.get_temperature(0), sim.get_necrosis(0), osim)
+    sim.close()
+
+
+def test_edge_cases(rfa, oracle):
+    table = W.tissue_table()
+    # zero steps, 1x1x1, tiny grids, single plane
+    for dims in ((1, 1, 1), (4, 4, 4), (8, 3, 2), (64, 64, 4), (4, 70, 9)):
+        nx, ny, nz = dims
+        rng = np.random.default_rng(nx * 100 + ny * 10 + nz)
+        lab = rng.integers(0, 7, size=(nz, ny, nx)).astype(np.uint8)
+        T0 = (37.0 + 30.0 * rng.random((nz, ny, nx))).astype(np.float32)
+        osim = oracle.OracleSim(dims, (1.0, 0.8, 1.2), lab, table, 37.0, 0.05)
+        osim.set_temperature(T0.astype(np.float64))
+        sim = rfa.RfaSim(dims, (1.0, 0.8, 1.2), lab, table, 37.0, 0.05)
+        sim.set_temperature(0, T0)
+        sim.step(0)
+        assert np.max(np.abs(sim.get_temperature(0) - T0)) < 4e-6      # theta = T - 37 round trip
+        sim.step(13)
+        osim.step(13)
+        compare(sim.get_temperature(0), sim.get_necrosis(0), osim)
+        sim.close()
+    with pytest.raises(rfa.RfaError):
+        rfa.RfaSim((4, 4, 4), (1, 1, 1), np.full((4, 4, 4), 9, np.uint8), table, 37.0, 0.1)
+    with pytest.raises(rfa.RfaError) as ei:
+        rfa.RfaSim((4, 4, 4), (0.5, 0.5, 0.5), np.ones((4, 4, 4), np.uint8), table, 37.0, 0.4)
+    assert ei.value.code == rfa.RFA_E_UNSTABLE
+    sim = rfa.RfaSim((4, 4, 4), (1, 1, 1), np.ones((4, 4, 4), np.uint8), table, 37.0, 0.1, batch=2)
+    with pytest.raises(rfa.RfaError):
+        sim.get_temperature(2)
+    with pytest.raises(rfa.RfaError):
+        sim.step(-1)
+    sim.close()
+
+
+def test_device_pointers_are_accepted(rfa):
+    import torch
+    w = W.ragged_phantom(dims=(44, 38, 29), steps=20)
+    sim = rfa.from_workload(w)
+    sim.step(20)
+    host = sim.get_temperature(0)
+    dev = torch.empty(host.shape, dtype=torch.float32, device="cuda")
+    sim.get_temperature(0, out=dev)
+    assert np.array_equal(dev.cpu().numpy(), host)
+    ndev = torch.empty(host.shape, dtype=torch.uint8, device="cuda")
+    sim.get_necrosis(0, out=ndev)
+    assert np.array_equal(ndev.cpu().numpy(), sim.get_necrosis(0))
+    # device-resident mask and temperature inputs
+    sim2 = rfa.RfaSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt)
+    sim2.set_needle(0, torch.from_numpy(w.needles[0].mask).cuda(), w.needles[0].mode, w.needles[0].value)
+    sim2.step(20)
+    assert np.array_equal(sim2.get_temperature(0), host)
+    sim2.set_temperature(0, dev)
+    assert np.max(np.abs(sim2.get_temperature(0) - host)) < 4e-6
+    sim.close()
+    sim2.close()
+
+
+# ----------------------------------------------------------------------------------------------
+# C1 (BASELINE configs[0]) incl. the Green's function variant, and invariants on the GPU field
+# ----------------------------------------------------------------------------------------------
+def test_c1_cube_and_green(rfa, oracle):
+    w = W.c1_cube()
+    osim = oracle.run_workload(w)
+    T, N, q = run_gpu(rfa, w, w.steps)
+    assert q["kernel"] == rfa.KERNEL_BLOCKED
+    err, _ = compare(T[0], N[0], osim)
+    # 48-fold symmetry survives fp32 exactly for the axis flips about the tip on this grid
+    c = 32
+    assert T[0][c, c, c + 3] == T[0][c, c, c - 3] == T[0][c + 3, c, c] == T[0][c, c - 3, c]
+    wg = W.c1_green(n=64, h_mm=1.0, dt=0.1, steps=1000)
+    og = oracle.run_workload(wg)
+    Tg, Ng, _ = run_gpu(rfa, wg, wg.steps)
+    # the delta start (37 + 1e4 C) is outside fp32's 1e-3 resolution at t=0; after 1000 steps it is smooth
+    compare(Tg[0], Ng[0], og, tol=2e-3)
+    # energy conservation on the GPU field (zero flux, no perfusion): sum(theta) constant
+    assert abs((Tg[0].astype(np.float64) - 37.0).sum() - 1.0e4) / 1.0e4 < 1e-4
+
+
+def test_monotone_and_bounded_on_gpu(rfa):
+    w = W.c2_phantom(steps=0)
+    sim = rfa.from_workload(w)
+    prev = sim.get_temperature(0)
+    prev_n = sim.necrotic_voxels(0)[0]
+    for _ in range(6):
+        sim.step(50)
+        cur = sim.get_temperature(0)
+        assert np.all(cur >= prev)                       # PAPER.md:83,:159 (fp32: exact here, monotone map)
+        assert cur.min() >= 37.0 and cur.max() <= 90.0
+        n = sim.necrotic_voxels(0)[0]
+        assert n >= prev_n
+        prev, prev_n = cur, n
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------
+# Full-length configs against the stored oracle results (tests/golden/, written by make_golden.py)
+# ----------------------------------------------------------------------------------------------
+def _golden(name):
+    path = os.path.join(GOLDEN, f"{name}_golden.npz")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated yet")
+    return np.load(path)
+
+
+def _check_against_golden(g, prefix, T, N, dims, idx_cp=-1):
+    nx, ny, nz = dims
+    idx = g[prefix + "sample_idx"]
+    exp = g[prefix + "sample_T"][idx_cp]
+    err = float(np.max(np.abs(T.ravel()[idx].astype(np.float64) - exp)))
+    assert err <= TOL, f"sampled max |dT| = {err:.3e}"
+    return err
+
+
+def _check_final_golden(g, prefix, T, N):
+    lo = g[prefix + "crop_lo"]
+    cT = g[prefix + "crop_T"]
+    c = cT.shape[0]
+    sub = T[lo[0]:lo[0] + c, lo[1]:lo[1] + c, lo[2]:lo[2] + c].astype(np.float64)
+    err = float(np.max(np.abs(sub - cT)))
+    assert err <= TOL, f"crop max |dT| = {err:.3e}"
+    No = np.unpackbits(g[prefix + "necro_packed"])[:N.size].reshape(N.shape)
+    mism = np.nonzero((N != 0).ravel() != (No != 0).ravel())[0]
+    band = g[prefix + "band_idx"][np.abs(g[prefix + "band_T"] - 60.0) <= BAND]
+    bad = np.setdiff1d(mism, band)
+    assert bad.size == 0, f"{bad.size} necrosis mismatches outside the band"
+    assert abs(float(T.astype(np.float64).max()) - float(g[prefix + "T_max"])) <= TOL
+    return err, int(mism.size)
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_full_length_config_vs_golden(rfa, name):
+    g = _golden(name)
+    w = W.BENCH_CONFIGS[name]()
+    from tests.golden.make_golden import fingerprint
+    assert fingerprint(w, 0) == str(g["fingerprint"]), "inputs differ from the ones the golden file was made from"
+    sim = rfa.from_workload(w)                    # default configuration = what bench.py times
+    done = 0
+    for ci, cp in enumerate(g["checkpoints"]):
+        sim.step(int(cp) - done)
+        done = int(cp)
+        T = sim.get_temperature(0)
+        _check_against_golden(g, "", T, None, w.dims, ci)
+    N = sim.get_necrosis(0)
+    err, n_mism = _check_final_golden(g, "", T, N)
+    all_v, tissue_v = sim.necrotic_voxels(0)
+    assert abs(all_v - int(g["necro_count"])) <= n_mism and abs(tissue_v - int(g["necro_count_tissue"])) <= n_mism
+    print(f"{name}: crop max|dT| {err:.2e}, necrosis mismatches (all inside the band) {n_mism}, "
+          f"necrotic voxels {all_v} (oracle {int(g['necro_count'])})")
+    sim.close()
+
+
+def test_c5_sweep_vs_golden(rfa):
+    g = _golden("C5")
+    w = W.c5_sweep()
+    from tests.golden.make_golden import fingerprint
+    sim = rfa.from_workload(w)
+    sim.step(w.steps)
+    vox = w.spacing_mm[0] * w.spacing_mm[1] * w.spacing_mm[2]
+    for b in range(w.batch):
+        p = f"s{b}_"
+        assert fingerprint(w, b) == str(g[p + "fingerprint"])
+        T = sim.get_temperature(b)
+        N = sim.get_necrosis(b)
+        _check_against_golden(g, p, T, N, w.dims)
+        err, n_mism = _check_final_golden(g, p, T, N)
+        _, tissue_v = sim.necrotic_voxels(b)
+        assert abs(tissue_v * vox - float(g[p + "necro_volume_mm3"])) <= n_mism * vox
+    sim.close()
