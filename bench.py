@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the RFA bioheat hot path (BASELINE.json: GVoxel-updates/s and
+simulated steps/s at 512x512x256, % of the B200 HBM roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
+
+A "step" is ONE simulated time step of the whole hot path (load, second
+differences, parameter lookup, source/sink, Euler update / hold, fused necrosis, buffer swap) over the
+whole synthetic volume.  K steps are issued as ONE ``rfa_step(K)`` call through the C ABI (the library
+fuses S steps per launch) and timed with CUDA events on the stream the kernels run on.
+
+Legs of one run (ours):
+  value     device-resident: state already in HBM, events around rfa_step(K)
+  e2e       whole job through the public API from pinned HOST buffers: rfa_create (labels H2D),
+            rfa_set_needle (mask H2D), rfa_step(K), rfa_get_temperature + rfa_get_necrosis (D2H),
+            host clock around all of it (create's allocation included)
+  roofline  dominant kernel: algorithmic bytes per launch / average launch duration over the timed region
+  cpu_baseline  the fp64 oracle (oracle/, as it stands) on the host cores, on a bounded sample (rank 0, N=1)
+
+N > 1 ("replicas only"): every rank runs an independent replica of the workload on
+its own GPU, no data-path collective; value = all ranks' voxel-updates / max-over-ranks time.
+
+``--impl reference`` times the oracle itself (there is no reference implementation to install: the
+reference is the paper text) on a bounded z-slab sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "GVoxel-updates/s"
+STATE_BYTES_PER_VOXEL_PASS = 9.0     # 4 B theta read + 4 B theta write + 1 B packed state read
+FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ----------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ----------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU every ~50 ms in a thread (NVML)."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = index
+            if vis:
+                ids = [v for v in vis.split(",") if v.strip()]
+                if index < len(ids) and ids[index].strip().isdigit():
+                    phys = int(ids[index])
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------------------------
+# multi-rank plumbing (one process per GPU; replicas only -- no data-path collective)
+# ----------------------------------------------------------------------------------------------
+def aggregate(local_ms: float, local_units: float, dist=None, device=None):
+    """(max over ranks of the time, sum over ranks of the units).  Works with any backend; unit-tested
+    with gloo / world_size 2 on CPU."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_ms, local_units
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ----------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference).  The only place bench.py touches oracle/.
+# ----------------------------------------------------------------------------------------------
+def _needle_slab(w, nzc):
+    """z-slab of nzc planes of workload w centred on the needle (inputs only; no method arithmetic)."""
+    nx, ny, nz = w.dims
+    nzc = int(max(1, min(nz, nzc)))
+    zc = int(round(np.nonzero(w.needles[0].mask)[0].mean())) if w.needles else nz // 2
+    z0 = int(min(max(zc - nzc // 2, 0), nz - nzc))
+    return z0, nzc
+
+
+def oracle_time(w, steps, warmup, nzc):
+    """Times `steps` oracle time steps on a z-slab of w (full slab = whole volume when nzc >= nz)."""
+    from oracle import rfa_oracle
+    rfa_oracle.build()
+    nx, ny, nz = w.dims
+    z0, nzc = _needle_slab(w, nzc)
+    sim = rfa_oracle.OracleSim((nx, ny, nzc), w.spacing_mm, w.labels[z0:z0 + nzc], w.table, w.t_blood, w.dt)
+    if w.needles:
+        nd = w.needles[0]
+        sim.set_needle(nd.mask[z0:z0 + nzc], nd.mode, nd.value)
+    if warmup:
+        sim.step(warmup)
+    t0 = time.perf_counter()
+    sim.step(steps)
+    secs = time.perf_counter() - t0
+    return secs, nx * ny * nzc, rfa_oracle.num_threads(), (z0, nzc)
+
+
+def cpu_baseline(w, budget_s=15.0):
+    """The oracle, as it stands, on a bounded sample: whole volume, as many time steps as fit ~budget_s."""
+    secs1, nv, thr, _ = oracle_time(w, 1, 0, w.dims[2])
+    n = int(max(1, min(50, budget_s / max(secs1, 1e-3))))
+    secs, nv, thr, _ = oracle_time(w, n, 0, w.dims[2])
+    gv = nv * n / secs / 1e9
+    return {"value": gv, "unit": METRIC, "cores": thr, "kind": "oracle",
+            "sample": f"{n} time steps of the full {w.dims[0]}x{w.dims[1]}x{w.dims[2]} {w.name} volume, fp64, "
+                      f"OpenMP over z ({secs:.1f} s)",
+            "steps_per_s": n / secs}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_1907_05709_b200 import workloads as W
+    w = W.BENCH_CONFIGS[args.config]()
+    nx, ny, nz = w.dims
+    # calibrate on a thin slab, then size the slab so K + W steps end within ~budget seconds
+    secs, nv, thr, _ = oracle_time(w, 2, 1, min(nz, 8))
+    rate = nv * 2 / secs
+    budget = 100.0
+    nzc = int(max(1, min(nz, budget * rate / ((args.steps + args.warmup) * nx * ny))))
+    secs, nv, thr, (z0, nzc) = oracle_time(w, args.steps, args.warmup, nzc)
+    gv = nv * args.steps / secs / 1e9
+    sample = (f"{args.steps} time steps on the z-slab [{z0},{z0 + nzc}) of {w.name} ({nx}x{ny}x{nzc} voxels around "
+              f"the needle), fp64 oracle, OpenMP over z")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gv, "unit": METRIC, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs * 1e3 / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "dims": [nx, ny, nz], "sample_dims": [nx, ny, nzc],
+                   "note": "the reference is the paper text only (no code); this arm times the repo's fp64 CPU oracle"},
+        "cpu_baseline": {"value": gv, "unit": METRIC, "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gv, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------
+def pinned(a):
+    """Copy a numpy array into pinned host memory (torch is used for the allocation only)."""
+    import torch
+    t = torch.empty(a.shape, dtype=torch.from_numpy(np.empty(0, a.dtype)).dtype, pin_memory=True)
+    v = t.numpy()
+    v[...] = a
+    return t, v
+
+
+def run_ours(args):
+    import torch
+    from paper_1907_05709_b200 import binding, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: librfa has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    binding.load_library()                      # raises if librfa.so is missing
+
+    w = W.BENCH_CONFIGS[args.config]()
+    nx, ny, nz = w.dims
+    nvox_all = w.n_voxels * w.batch
+    K, Wu = args.steps, args.warmup
+    stream = torch.cuda.Stream(device=dev)
+
+    # ---- device-resident leg ------------------------------------------------------------------
+    with torch.cuda.stream(stream):
+        sim = binding.from_workload(w, device=dev, stream=stream)
+        sim.configure(args.kernel, args.fused)
+        sim.step(Wu)
+        sim.synchronize()
+        q0 = sim.query()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+        with ClockSampler(local) as clk:
+            e0.record(stream)
+            sim.step(K)
+            e1.record(stream)
+            e1.synchronize()
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+        ms_local = float(e0.elapsed_time(e1))
+        q1 = sim.query()
+        necro_all, necro_tissue = sim.necrotic_voxels(0)
+        tmax = float(sim.get_temperature(0).max())
+        sim.close()
+        del sim
+    launches = q1["kernel_launches"] - q0["kernel_launches"]
+    ms, units = aggregate(ms_local, float(nvox_all) * K, dist, dev)
+    gvox = units / (ms * 1e-3) / 1e9
+    peak, peak_src = measured_peak()
+
+    # dominant kernel = the stepping kernel: the timed region holds nothing else on this stream
+    launch_us = ms_local * 1e3 / max(launches, 1)
+    bytes_per_launch = STATE_BYTES_PER_VOXEL_PASS * nvox_all
+    achieved = bytes_per_launch / (launch_us * 1e-6) / 1e9
+    roofline = {
+        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": None, "peak_source": peak_src,
+        "kernel": f"rfa_blocked_kernel<S={q1['fused_steps']}>" if q1["kernel"] == binding.KERNEL_BLOCKED else "rfa_plain_kernel",
+        "launches": launches, "avg_launch_us": launch_us, "algorithmic_bytes_per_launch": bytes_per_launch,
+        "fused_steps_per_launch": q1["fused_steps"],
+        # north_star's roofline-equivalent: one 4-B read + one 4-B write of the field per *time step*
+        "equiv_8B_frac": gvox / world * 8.0 / peak,
+    }
+
+    # ---- end-to-end leg: host buffers in, host buffers out --------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        _, lab_h = pinned(np.ascontiguousarray(w.labels, dtype=np.uint8))
+        masks = [pinned(np.ascontiguousarray(nd.mask, dtype=np.uint8))[1] for nd in w.needles]
+        _, T_h = pinned(np.empty((nz, ny, nx), np.float32))
+        _, N_h = pinned(np.empty((nz, ny, nx), np.uint8))
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        with torch.cuda.stream(stream):
+            s2 = binding.RfaSim(w.dims, w.spacing_mm, lab_h, w.table, w.t_blood, w.dt, batch=w.batch,
+                                device=dev, stream=stream)
+            s2.configure(args.kernel, args.fused)
+            for b, nd in enumerate(w.needles):
+                s2.set_needle(b, masks[b], nd.mode, nd.value, nd.tip_mm, nd.axis)
+            s2.step(K)
+            for b in range(w.batch):
+                s2.get_temperature(b, out=T_h)
+                s2.get_necrosis(b, out=N_h)
+            s2.synchronize()
+        torch.cuda.synchronize(dev)
+        e2e_ms_local = (time.perf_counter() - t0) * 1e3
+        s2.close()
+        e2e_ms, e2e_units = aggregate(e2e_ms_local, float(nvox_all) * K, dist, dev)
+        h2d = w.n_voxels * (1 + len(w.needles))
+        d2h = w.n_voxels * 5 * w.batch
+        e2e = {"value": e2e_units / (e2e_ms * 1e-3) / 1e9, "unit": METRIC,
+               "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+               "h2d_bytes_per_job": h2d, "d2h_bytes_per_job": d2h, "job_ms": e2e_ms,
+               "what": "rfa_create(host labels) + rfa_set_needle(host mask) + rfa_step(K) + rfa_get_temperature/"
+                       "rfa_get_necrosis into pinned host buffers, host clock, allocation included"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(w)
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": gvox, "unit": METRIC, "n_gpus": world, "steps": K, "warmup": Wu,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "dims": [nx, ny, nz], "batch": w.batch, "spacing_mm": list(w.spacing_mm),
+                       "dt_s": w.dt, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (2 x %d MiB fields + %d MiB state vs 126 MB L2)" % (
+                           nvox_all * 4 >> 20, nvox_all >> 20) if nvox_all * 9 > 126e6 * 2 else
+                             "working set fits L2 (reported, not held to the HBM bar)",
+                       "kernel": roofline["kernel"]},
+            "sim_steps_per_s": K / (ms * 1e-3) * (1 if world == 1 else world),
+            "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
+            "clocks": clk.summary(),
+            "check": {"t_max_c": tmax, "necrotic_voxels": necro_all, "necrotic_tissue_voxels": necro_tissue},
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=12000)
+    ap.add_argument("--warmup", type=int, default=120)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 plain, 2 blocked (rfa_configure)")
+    ap.add_argument("--fused", type=int, default=0, help="fused time steps per launch, 0 = library default")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args(argv)
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
