@@ -129,8 +129,8 @@ int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launche
 
 /* Host-only view of the blocked kernel's launch plan for a grid (no GPU needed; used by the unit tests
  * and the bench report).  resident_ctas = CTAs that can be co-resident (SM count x occupancy).
- * out = { ok, tiles_x, tiles_y, z_chunks, planes_per_chunk, work_items, ctas_launched }. */
-int rfa_plan_query(const int dims[3], int batch, int fused_steps, int resident_ctas, int out[7]);
+ * out = { ok, tiles_x, tiles_y, z_chunks, planes_per_chunk, work_items, ctas_launched, tile_bx, tile_by }. */
+int rfa_plan_query(const int dims[3], int batch, int fused_steps, int resident_ctas, int out[9]);
 
 int rfa_synchronize(rfa_sim *s);
 void rfa_destroy(rfa_sim *s);

@@ -12,7 +12,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "librfa.so")
+# RFA_LIBRARY lets a developer load another build of the same library (e.g. a tile-shape experiment)
+LIB_PATH = os.environ.get("RFA_LIBRARY") or os.path.join(_HERE, "librfa.so")
 
 RFA_OK, RFA_E_INVALID, RFA_E_UNSTABLE, RFA_E_CUDA, RFA_E_NOMEM = 0, -1, -2, -3, -4
 SRC_OFF, SRC_DIRICHLET, SRC_POWER = 0, 1, 2
@@ -120,9 +121,9 @@ def stability_number(spacing_mm, table, dt) -> float:
 
 def plan_query(dims, batch, fused, resident_ctas) -> dict:
     lib = load_library()
-    out = (ctypes.c_int * 7)()
+    out = (ctypes.c_int * 9)()
     _check(lib.rfa_plan_query(_i3(dims), int(batch), int(fused), int(resident_ctas), out))
-    keys = ["ok", "tiles_x", "tiles_y", "z_chunks", "planes_per_chunk", "work_items", "ctas"]
+    keys = ["ok", "tiles_x", "tiles_y", "z_chunks", "planes_per_chunk", "work_items", "ctas", "bx", "by"]
     return dict(zip(keys, [int(x) for x in out]))
 
 

@@ -144,11 +144,11 @@ static void build_table(const rfa_sim *s, double q_power, RfaTableHost &out)
             const rfa_tissue &t = s->table[l];
             const double kw = (double)t.k * W;
             a = s->dt / ((double)t.rho * t.cp) * kw;
-            nk = -(2.0 + (double)t.wb_cb / kw);
+            nk = -(double)t.wb_cb / kw;
             qa = ((double)t.q_m + (pow ? q_power : 0.0)) / kw;
         }
         out.a[e] = (float)a;
-        out.nk[e] = (float)nk;
+        out.np[e] = (float)nk;
         out.qa[e] = (float)qa;
     }
 }
@@ -162,7 +162,7 @@ RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int res
     p.fused = fused;
     const int S = fused;
     if (S < 1 || S > 4 || nx < 4 || (nx % 4) != 0 || ny < S || nz < S || batch < 1 || resident_ctas < 1) return p;
-    const int BX = RFA_TB_BX, BY = RFA_TB_BY;
+    const int BX = 4 * RFA_TB_SHAPE[S].tx, BY = RFA_TB_SHAPE[S].ry * RFA_TB_SHAPE[S].ty;
     p.tiles_x = nx <= BX ? 1 : (nx - 8 + (BX - 8) - 1) / (BX - 8);
     p.tiles_y = (ny + (BY - 2 * S) - 1) / (BY - 2 * S);
     const long long per_z = (long long)p.tiles_x * p.tiles_y * batch;
@@ -189,7 +189,7 @@ RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int res
 }
 
 // exported for the CPU unit tests of the planner (no GPU needed)
-extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resident_ctas, int out[7])
+extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resident_ctas, int out[9])
 {
     if (!dims || !out) return RFA_E_INVALID;
     RfaTbPlan p = rfa_plan_blocked(dims[0], dims[1], dims[2], batch, fused, resident_ctas);
@@ -200,6 +200,8 @@ extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resid
     out[4] = p.zchunk;
     out[5] = p.n_items;
     out[6] = p.grid;
+    out[7] = p.ok ? 4 * RFA_TB_SHAPE[fused].tx : 0;
+    out[8] = p.ok ? RFA_TB_SHAPE[fused].ry * RFA_TB_SHAPE[fused].ty : 0;
     return RFA_OK;
 }
 
@@ -291,9 +293,21 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
         s->h_m[a] = (double)spacing_mm[a] * 1.0e-3;          // mm -> m (PAPER.md:115 vs :104)
         W += 1.0 / (s->h_m[a] * s->h_m[a]);
     }
-    s->g.wx = (float)(1.0 / (s->h_m[0] * s->h_m[0]) / W);
-    s->g.wy = (float)(1.0 / (s->h_m[1] * s->h_m[1]) / W);
-    s->g.wz = (float)(1.0 / (s->h_m[2] * s->h_m[2]) / W);
+    {
+        // weights on the 2^-24 grid with an exact unit sum (rfa_device.cuh); the largest absorbs the residue
+        const double q = 16777216.0;
+        double w[3], wq[3];
+        int big = 0;
+        for (int a = 0; a < 3; ++a) {
+            w[a] = 1.0 / (s->h_m[a] * s->h_m[a]) / W;
+            wq[a] = std::nearbyint(w[a] * q) / q;
+            if (w[a] > w[big]) big = a;
+        }
+        wq[big] = 1.0 - wq[(big + 1) % 3] - wq[(big + 2) % 3];
+        s->g.wx = (float)wq[0];
+        s->g.wy = (float)wq[1];
+        s->g.wz = (float)wq[2];
+    }
     s->dt = dt_s;
     s->t_blood = t_blood_c;
     s->g.t_blood = t_blood_c;

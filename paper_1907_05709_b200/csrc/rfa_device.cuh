@@ -20,28 +20,34 @@
 // Per-scenario coefficient table, three planes of RFA_TABLE_N floats each (fp64 on the host,
 // rounded once):
 //   a[e]   = dt K /(rho c_p) * W          W = 1/dx^2 + 1/dy^2 + 1/dz^2 (metres)      (0 for held entries)
-//   nk[e]  = -(2 + w_b c_b /(K W))        (0 for held entries)
+//   np[e]  = -w_b c_b /(K W)              (0 for held entries)
 //   qa[e]  = (Q_m + Q_power) / (K W)      (0 for held entries)
-// and three global weights wx = (1/dx^2)/W, wy, wz.
+// and three global weights wx = (1/dx^2)/W, wy, wz, rounded to multiples of 2^-24 such that their
+// fp32 values sum to exactly 1 (otherwise the cancellation
+// wx sx + wy sy + wz sz - 2 theta leaves a systematic source ~ 1e-7 * 2 theta per step).
 struct RfaTableHost {
     float a[RFA_TABLE_N];
-    float nk[RFA_TABLE_N];
+    float np[RFA_TABLE_N];
     float qa[RFA_TABLE_N];
 };
 
 // theta' for one voxel.  theta = T - T_a.  Eq. 12 rearranged as
-//   theta' = theta + a * ( wx (xm+xp) + wy (ym+yp) + wz (zm+zp) + qa - (2 + p/a) theta )
-// Explicit intrinsics fix the rounding sequence, so every kernel variant is bit-identical.
+//   theta' = theta + a * ( wx (xm+xp) + wy (ym+yp) + wz (zm+zp) - 2 theta + qa - (p/a) theta )
+// The "-2 theta" is applied with the exact constant 2 and the perfusion term separately, so no
+// rounded coefficient multiplies the large cancelling terms.  Explicit intrinsics fix the rounding
+// sequence, so every kernel variant is bit-identical (the blocked kernel evaluates the same sequence
+// two voxels at a time with add.rn.f32x2 / fma.rn.f32x2).
 // A held voxel has a = 0 and returns theta exactly (Eq. 13, Alg. 1 :313).
 __device__ __forceinline__ float rfa_update(float t, float xm, float xp, float ym, float yp, float zm,
-                                            float zp, float a, float nk, float qa, float wx, float wy,
+                                            float zp, float a, float np, float qa, float wx, float wy,
                                             float wz)
 {
     const float sx = __fadd_rn(xm, xp);
     const float sy = __fadd_rn(ym, yp);
     const float sz = __fadd_rn(zm, zp);
-    const float l = __fmaf_rn(wz, sz, __fmaf_rn(wy, sy, __fmaf_rn(wx, sx, qa)));
-    const float g = __fmaf_rn(nk, t, l);
+    const float u = __fmaf_rn(np, t, qa);
+    const float l = __fmaf_rn(wz, sz, __fmaf_rn(wy, sy, __fmaf_rn(wx, sx, u)));
+    const float g = __fmaf_rn(-2.0f, t, l);
     return __fmaf_rn(a, g, t);
 }
 

@@ -24,8 +24,39 @@ struct RfaTbPlan {
     int ok;                    // 0: this grid cannot use the blocked kernel
 };
 
-// tile constants of the blocked kernel (one configuration in round 1)
-enum { RFA_TB_TX = 16, RFA_TB_TY = 16, RFA_TB_RY = 4, RFA_TB_BX = 4 * RFA_TB_TX, RFA_TB_BY = RFA_TB_RY * RFA_TB_TY };
+// tile shape of the blocked kernel per number of fused steps S (index 1..4): TX x TY threads, each owning
+// one float4 column and RY rows -> BX = 4 TX by BY = RY TY voxels per plane; minb = CTAs per SM asked
+// of the compiler (register cap).
+struct RfaTbShape {
+    int tx, ty, ry, minb;
+};
+#ifndef RFA_TX
+#define RFA_TX 16
+#endif
+#ifndef RFA_TY
+#define RFA_TY 16
+#endif
+#ifndef RFA_S1_RY
+#define RFA_S1_RY 4
+#define RFA_S1_MINB 2
+#endif
+#ifndef RFA_S2_RY
+#define RFA_S2_RY 2
+#define RFA_S2_MINB 2
+#endif
+#ifndef RFA_S3_RY
+#define RFA_S3_RY 2
+#define RFA_S3_MINB 2
+#endif
+#ifndef RFA_S4_RY
+#define RFA_S4_RY 2
+#define RFA_S4_MINB 2
+#endif
+constexpr RfaTbShape RFA_TB_SHAPE[5] = {{0, 0, 0, 0},
+                                        {RFA_TX, RFA_TY, RFA_S1_RY, RFA_S1_MINB},
+                                        {RFA_TX, RFA_TY, RFA_S2_RY, RFA_S2_MINB},
+                                        {RFA_TX, RFA_TY, RFA_S3_RY, RFA_S3_MINB},
+                                        {RFA_TX, RFA_TY, RFA_S4_RY, RFA_S4_MINB}};
 
 // host-only planning (no CUDA calls): implemented in rfa_api.cpp, unit-tested on CPU
 RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int resident_ctas);

@@ -38,7 +38,7 @@ __global__ void rfa_table_kernel(RfaTableHost tbl, float *dst)
     int e = threadIdx.x;
     if (e < RFA_TABLE_N) {
         dst[e] = tbl.a[e];
-        dst[RFA_TABLE_N + e] = tbl.nk[e];
+        dst[RFA_TABLE_N + e] = tbl.np[e];
         dst[2 * RFA_TABLE_N + e] = tbl.qa[e];
     }
 }
@@ -164,11 +164,19 @@ __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float
 // ------------------------------------------------------------------------------------------------
 // Work item = (scenario, z chunk, y tile, x tile); a CTA of TX*TY threads owns a BX x BY xy tile
 // (BX = 4 TX, BY = RY TY) and streams it along z.  Thread (tx,ty) owns the float4 column tx and the
-// RY rows ty*RY.. of every plane.  For each fused level k = 1..S it keeps the previous and the centre
-// plane of level k-1 in registers (the z queue); the next plane arrives from level k-1 in the same
-// iteration, level 0 being the plane just landed from HBM (cp.async ring, thread-private slots).
+// RY rows ty*RY.. of every plane.  For each fused level k = 0..S-1 it keeps three planes of level k in
+// registers (slots rotate with the iteration number mod 3; the plane loop is unrolled three times so
+// the rotation costs no register moves): the plane that arrived this iteration (z+1), the centre
+// plane (z) and the previous one (z-1).  Level 0 arrives from HBM through a thread-private cp.async
+// ring; level k+1 of the centre plane is produced in the same iteration and is level k+1's arrival.
 // x neighbours come from warp shuffles, y neighbours across threads from a double-buffered shared
 // exchange of each thread's first/last row -> one __syncthreads per plane.
+//
+// Arithmetic: the same rounding sequence as rfa_update(), evaluated two voxels at a time with the
+// packed fp32 instructions of sm_100 (add.rn.f32x2 / fma.rn.f32x2 -> FADD2 / FFMA2), so the result is
+// bit-identical to the plain kernel.  Coefficients: when all RY*4 voxels of every thread of the warp
+// carry one label (the common case away from tissue interfaces) they are fetched once per thread and
+// level; otherwise once per voxel.
 //
 // Halos: x tiles overlap by 8 columns (4 = one float4 per side, S <= 4), y tiles and z chunks carry
 // S halo rows / planes per side.  At the outer y and z faces the halo is loaded MIRRORED
@@ -191,9 +199,9 @@ struct TbCfg {
     static constexpr int NT = TX * TY;
     static constexpr int BX = 4 * TX;
     static constexpr int BY = RY * TY;
-    static constexpr int PD = 2;              // prefetch distance (planes in flight)
+    static constexpr int PD = 1;              // prefetch distance (planes in flight)
     static constexpr int DT = PD + 1;         // temperature ring depth
-    static constexpr int DS = PD + S + 1;     // state ring depth (level k reads plane i-k)
+    static constexpr int DS = PD + S + 1;     // state ring depth (level k reads plane i-k-1)
     static constexpr size_t RING_T = (size_t)DT * RY * NT * 16;
     static constexpr size_t EXCH = (size_t)S * 2 * 2 * NT * 16;
     static constexpr size_t RING_S = (size_t)DS * RY * NT * 4;
@@ -201,15 +209,42 @@ struct TbCfg {
     static constexpr size_t SMEM = RING_T + EXCH + RING_S + TAB;
 };
 
-template <int S, int TX, int TY, int RY>
-__global__ void __launch_bounds__(TX *TY, 1) rfa_blocked_kernel(const RfaTbParams P)
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk(float lo, float hi)
+{
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk(u64 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ u64 add2(u64 a, u64 b)
+{
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
+{
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+template <int I>
+struct IC {
+    static constexpr int value = I;
+};
+
+template <int S, int TX, int TY, int RY, int MINB>
+__global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbParams P)
 {
     using C = TbCfg<S, TX, TY, RY>;
     constexpr int NT = C::NT, BX = C::BX, BY = C::BY, PD = C::PD, DT = C::DT, DS = C::DS;
+    static_assert(RY == 4 || RY == 2, "state words of a thread are read as one vector");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *ringT = reinterpret_cast<float4 *>(smem_raw);                  // [DT][RY][NT]
     float4 *exch = reinterpret_cast<float4 *>(smem_raw + C::RING_T);       // [S][2 parity][2 top/bot][NT]
-    uint32_t *ringS = reinterpret_cast<uint32_t *>(smem_raw + C::RING_T + C::EXCH);   // [DS][RY][NT]
+    uint32_t *ringS = reinterpret_cast<uint32_t *>(smem_raw + C::RING_T + C::EXCH);   // [DS][NT][RY]
     float *tab = reinterpret_cast<float *>(smem_raw + C::RING_T + C::EXCH + C::RING_S);   // [3][128]
 
     const int tid = threadIdx.x;
@@ -220,6 +255,8 @@ __global__ void __launch_bounds__(TX *TY, 1) rfa_blocked_kernel(const RfaTbParam
     for (int e = tid; e < S * 2 * 2 * NT; e += NT) exch[e] = make_float4(0.f, 0.f, 0.f, 0.f);
 
     const size_t plane4 = (size_t)P.ny * P.nx4;       // float4 (= state words) per plane
+    const u64 wx2 = pk(P.wx, P.wx), wy2 = pk(P.wy, P.wy), wz2 = pk(P.wz, P.wz), m2 = pk(-2.0f, -2.0f);
+    const float thr = P.thr;
     int cur_b = -1;
 
     for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
@@ -241,14 +278,14 @@ __global__ void __launch_bounds__(TX *TY, 1) rfa_blocked_kernel(const RfaTbParam
         const bool xr_self = (gx4 == P.nx4 - 1);
         const bool col_ok = (gx4 < P.nx4) && !(tx == 0 && X0 > 0) && !(tx == TX - 1 && X0 + BX < P.nx);
         unsigned row_ok = 0;
-        size_t row_src[RY], row_dst[RY];
+        unsigned row_src[RY], row_dst[RY];               // float4 offsets inside one plane
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
             const int ly = ty * RY + r;
             const int gy = Y0 + ly;
             if (ly >= S && ly < BY - S && gy >= 0 && gy < P.ny && col_ok) row_ok |= 1u << r;
-            row_src[r] = (size_t)rfa_reflect(gy, P.ny) * P.nx4 + gx4c;
-            row_dst[r] = (size_t)min(max(gy, 0), P.ny - 1) * P.nx4 + gx4c;
+            row_src[r] = (unsigned)(rfa_reflect(gy, P.ny) * P.nx4 + gx4c);
+            row_dst[r] = (unsigned)(min(max(gy, 0), P.ny - 1) * P.nx4 + gx4c);
         }
         const size_t base4 = (size_t)b * P.nz * plane4;
         const float4 *tin4 = reinterpret_cast<const float4 *>(P.tin) + base4;
@@ -261,17 +298,17 @@ __global__ void __launch_bounds__(TX *TY, 1) rfa_blocked_kernel(const RfaTbParam
             cur_b = b;
         }
 
-        float4 qm[S][RY], qc[S][RY];                       // z queue: previous / centre plane per level
-        unsigned nbc[S];                                   // necrosis bits travelling with qc
+        // q[k][slot][r]: three planes of level k (see the header comment); nbq: their necrosis bits
+        float4 q[S][3][RY];
+        unsigned nbq[S][3];
 #pragma unroll
-        for (int k = 0; k < S; ++k) {
-            nbc[k] = 0;
+        for (int k = 0; k < S; ++k)
 #pragma unroll
-            for (int r = 0; r < RY; ++r) {
-                qm[k][r] = make_float4(0.f, 0.f, 0.f, 0.f);
-                qc[k][r] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int s = 0; s < 3; ++s) {
+                nbq[k][s] = 0;
+#pragma unroll
+                for (int r = 0; r < RY; ++r) q[k][s][r] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
-        }
 
         const int niter = (z1 - z0) + 2 * S;
         auto issue = [&](int j) {
@@ -281,7 +318,7 @@ __global__ void __launch_bounds__(TX *TY, 1) rfa_blocked_kernel(const RfaTbParam
 #pragma unroll
             for (int r = 0; r < RY; ++r) {
                 cp_async16(&ringT[(sT * RY + r) * NT + tid], tin4 + pl + row_src[r]);
-                cp_async4(&ringS[(sS * RY + r) * NT + tid], st4 + pl + row_src[r]);
+                cp_async4(&ringS[(sS * NT + tid) * RY + r], st4 + pl + row_src[r]);
             }
         };
 #pragma unroll
@@ -290,83 +327,119 @@ __global__ void __launch_bounds__(TX *TY, 1) rfa_blocked_kernel(const RfaTbParam
             cp_async_commit();
         }
 
-        for (int i = 0; i < niter; ++i) {
+        // one plane iteration; PH = i mod 3 selects the register slots at compile time
+        auto body = [&](auto ph, const int i) {
+            constexpr int PH = decltype(ph)::value;
+            constexpr int CE = (PH + 2) % 3;               // centre plane slot
+            constexpr int MI = (PH + 1) % 3;               // previous plane slot
             if (i + PD < niter) issue(i + PD);
             cp_async_commit();
             cp_async_wait<PD>();
-            __syncthreads();                               // exchange rows of iteration i-1 are visible
-
-            const int par_w = i & 1, par_r = par_w ^ 1;
-            float4 in[RY];
-            unsigned nb_in = 0;
             {
                 const int sT = i % DT;
 #pragma unroll
-                for (int r = 0; r < RY; ++r) in[r] = ringT[(sT * RY + r) * NT + tid];
+                for (int r = 0; r < RY; ++r) q[0][PH][r] = ringT[(sT * RY + r) * NT + tid];
+                nbq[0][PH] = 0;
             }
+            __syncthreads();                               // exchange rows of iteration i-1 are visible
+            const int par_w = i & 1, par_r = par_w ^ 1;
+            float4 out[RY];
+            unsigned nb_out = 0;
 #pragma unroll
             for (int k = 0; k < S; ++k) {
-                // publish first/last row of level-k input plane (it is the centre plane next iteration)
-                exch[((k * 2 + par_w) * 2 + 0) * NT + tid] = in[0];
-                exch[((k * 2 + par_w) * 2 + 1) * NT + tid] = in[RY - 1];
+                // publish first/last row of the arriving level-k plane (it is the centre plane next iteration)
+                exch[((k * 2 + par_w) * 2 + 0) * NT + tid] = q[k][PH][0];
+                exch[((k * 2 + par_w) * 2 + 1) * NT + tid] = q[k][PH][RY - 1];
                 const float4 above = exch[((k * 2 + par_r) * 2 + 1) * NT + up_tid];
                 const float4 below = exch[((k * 2 + par_r) * 2 + 0) * NT + dn_tid];
-                const int sS = (i - (k + 1) + 2 * DS) % DS;          // state of plane zin-(k+1)
-                float4 o[RY];
+                int sS = i % DS - (k + 1);                  // state of the centre plane
+                if (sS < 0) sS += DS;
+                uint32_t sw[RY];
+                if constexpr (RY == 4) {
+                    const uint4 v = *reinterpret_cast<const uint4 *>(&ringS[(sS * NT + tid) * RY]);
+                    sw[0] = v.x; sw[1] = v.y; sw[2] = v.z; sw[3] = v.w;
+                } else {
+                    const uint2 v = *reinterpret_cast<const uint2 *>(&ringS[(sS * NT + tid) * RY]);
+                    sw[0] = v.x; sw[1] = v.y;
+                }
+                // one label for all voxels of every thread of the warp?
+                uint32_t diff = sw[0] ^ __byte_perm(sw[0], 0, 0);
+#pragma unroll
+                for (int r = 1; r < RY; ++r) diff |= sw[0] ^ sw[r];
+                const bool uni = __all_sync(0xffffffffu, (diff & 0x7f7f7f7fu) == 0u);
+                u64 a01, a23, n01, n23, q01, q23;
+                if (uni) {
+                    const unsigned e = sw[0] & RFA_ST_INDEX;
+                    const float a = tab[e], nk = tab[RFA_TABLE_N + e], qa = tab[2 * RFA_TABLE_N + e];
+                    a01 = a23 = pk(a, a);
+                    n01 = n23 = pk(nk, nk);
+                    q01 = q23 = pk(qa, qa);
+                }
                 float mx = -3.0e38f;
 #pragma unroll
                 for (int r = 0; r < RY; ++r) {
-                    const float4 c = qc[k][r];
-                    const float4 u = (r == 0) ? above : qc[k][r - 1];
-                    const float4 d = (r == RY - 1) ? below : qc[k][r + 1];
+                    const float4 c = q[k][CE][r];
+                    const float4 u = (r == 0) ? above : q[k][CE][r - 1];
+                    const float4 d = (r == RY - 1) ? below : q[k][CE][r + 1];
                     float left = __shfl_up_sync(0xffffffffu, c.w, 1, TX);
                     float right = __shfl_down_sync(0xffffffffu, c.x, 1, TX);
                     if (xl_self) left = c.x;               // zero flux at the outer x faces (R-7)
                     if (xr_self) right = c.w;
-                    const uint32_t w = ringS[(sS * RY + r) * NT + tid];
-                    const unsigned e0 = w & RFA_ST_INDEX, e1 = (w >> 8) & RFA_ST_INDEX,
-                                   e2 = (w >> 16) & RFA_ST_INDEX, e3 = (w >> 24) & RFA_ST_INDEX;
-                    const float4 zm = qm[k][r], zp = in[r];
-                    o[r].x = rfa_update(c.x, left, c.y, u.x, d.x, zm.x, zp.x, tab[e0], tab[RFA_TABLE_N + e0],
-                                        tab[2 * RFA_TABLE_N + e0], P.wx, P.wy, P.wz);
-                    o[r].y = rfa_update(c.y, c.x, c.z, u.y, d.y, zm.y, zp.y, tab[e1], tab[RFA_TABLE_N + e1],
-                                        tab[2 * RFA_TABLE_N + e1], P.wx, P.wy, P.wz);
-                    o[r].z = rfa_update(c.z, c.y, c.w, u.z, d.z, zm.z, zp.z, tab[e2], tab[RFA_TABLE_N + e2],
-                                        tab[2 * RFA_TABLE_N + e2], P.wx, P.wy, P.wz);
-                    o[r].w = rfa_update(c.w, c.z, right, u.w, d.w, zm.w, zp.w, tab[e3], tab[RFA_TABLE_N + e3],
-                                        tab[2 * RFA_TABLE_N + e3], P.wx, P.wy, P.wz);
-                    mx = fmaxf(mx, fmaxf(fmaxf(o[r].x, o[r].y), fmaxf(o[r].z, o[r].w)));
+                    if (!uni) {
+                        const uint32_t w = sw[r];
+                        const unsigned e0 = w & RFA_ST_INDEX, e1 = (w >> 8) & RFA_ST_INDEX,
+                                       e2 = (w >> 16) & RFA_ST_INDEX, e3 = (w >> 24) & RFA_ST_INDEX;
+                        a01 = pk(tab[e0], tab[e1]);
+                        a23 = pk(tab[e2], tab[e3]);
+                        n01 = pk(tab[RFA_TABLE_N + e0], tab[RFA_TABLE_N + e1]);
+                        n23 = pk(tab[RFA_TABLE_N + e2], tab[RFA_TABLE_N + e3]);
+                        q01 = pk(tab[2 * RFA_TABLE_N + e0], tab[2 * RFA_TABLE_N + e1]);
+                        q23 = pk(tab[2 * RFA_TABLE_N + e2], tab[2 * RFA_TABLE_N + e3]);
+                    }
+                    const float4 zm = q[k][MI][r], zp = q[k][PH][r];
+                    // same rounding sequence as rfa_update(), two voxels per instruction
+                    const u64 t01 = pk(c.x, c.y), t23 = pk(c.z, c.w);
+                    const u64 sx01 = pk(__fadd_rn(left, c.y), __fadd_rn(c.x, c.z));
+                    const u64 sx23 = pk(__fadd_rn(c.y, c.w), __fadd_rn(c.z, right));
+                    const u64 sy01 = add2(pk(u.x, u.y), pk(d.x, d.y)), sy23 = add2(pk(u.z, u.w), pk(d.z, d.w));
+                    const u64 sz01 = add2(pk(zm.x, zm.y), pk(zp.x, zp.y)), sz23 = add2(pk(zm.z, zm.w), pk(zp.z, zp.w));
+                    const u64 l01 = fma2(wz2, sz01, fma2(wy2, sy01, fma2(wx2, sx01, fma2(n01, t01, q01))));
+                    const u64 l23 = fma2(wz2, sz23, fma2(wy2, sy23, fma2(wx2, sx23, fma2(n23, t23, q23))));
+                    const u64 o01 = fma2(a01, fma2(m2, t01, l01), t01);
+                    const u64 o23 = fma2(a23, fma2(m2, t23, l23), t23);
+                    float4 o;
+                    upk(o01, o.x, o.y);
+                    upk(o23, o.z, o.w);
+                    mx = fmaxf(mx, fmaxf(fmaxf(o.x, o.y), fmaxf(o.z, o.w)));
+                    if (k + 1 < S) q[(k + 1) % S][PH][r] = o;
+                    else out[r] = o;
                 }
-                unsigned nb_o = nbc[k];
-                if (mx >= P.thr) {                         // rare: some voxel of this thread reached 60 C
+                unsigned nb_o = nbq[k][CE];
+                if (mx >= thr) {                           // rare: some voxel of this thread reached 60 C
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
-                        nb_o |= (o[r].x >= P.thr ? 1u : 0u) << (4 * r);
-                        nb_o |= (o[r].y >= P.thr ? 2u : 0u) << (4 * r);
-                        nb_o |= (o[r].z >= P.thr ? 4u : 0u) << (4 * r);
-                        nb_o |= (o[r].w >= P.thr ? 8u : 0u) << (4 * r);
+                        const float4 o = (k + 1 < S) ? q[(k + 1) % S][PH][r] : out[r];
+                        nb_o |= (o.x >= thr ? 1u : 0u) << (4 * r);
+                        nb_o |= (o.y >= thr ? 2u : 0u) << (4 * r);
+                        nb_o |= (o.z >= thr ? 4u : 0u) << (4 * r);
+                        nb_o |= (o.w >= thr ? 8u : 0u) << (4 * r);
                     }
                 }
-                nbc[k] = nb_in;
-                nb_in = nb_o;
-#pragma unroll
-                for (int r = 0; r < RY; ++r) {
-                    qm[k][r] = qc[k][r];
-                    qc[k][r] = in[r];
-                    in[r] = o[r];
-                }
+                if (k + 1 < S) nbq[(k + 1) % S][PH] = nb_o;
+                else nb_out = nb_o;
             }
-            // `in` is now level S of plane z0 + (i - 2S)
+            // `out` is level S of plane z0 + (i - 2S)
             if (i >= 2 * S) {
                 const size_t pl = (size_t)(z0 + i - 2 * S) * plane4;
-                const int sS = (i - S + 2 * DS) % DS;
+                int sS = i % DS - S;
+                if (sS < 0) sS += DS;
 #pragma unroll
                 for (int r = 0; r < RY; ++r) {
                     if (row_ok & (1u << r)) {
-                        tout4[pl + row_dst[r]] = in[r];
-                        const unsigned bits = (nb_in >> (4 * r)) & 0xfu;
+                        tout4[pl + row_dst[r]] = out[r];
+                        const unsigned bits = (nb_out >> (4 * r)) & 0xfu;
                         if (bits) {
-                            const uint32_t w = ringS[(sS * RY + r) * NT + tid];
+                            const uint32_t w = ringS[(sS * NT + tid) * RY + r];
                             const uint32_t nw = w | ((bits & 1u) << 7) | ((bits & 2u) << 14) | ((bits & 4u) << 21) |
                                                 ((bits & 8u) << 28);
                             if (nw != w) st4[pl + row_dst[r]] = nw;
@@ -374,6 +447,15 @@ __global__ void __launch_bounds__(TX *TY, 1) rfa_blocked_kernel(const RfaTbParam
                     }
                 }
             }
+        };
+
+        for (int i = 0;;) {
+            body(IC<0>{}, i);
+            if (++i >= niter) break;
+            body(IC<1>{}, i);
+            if (++i >= niter) break;
+            body(IC<2>{}, i);
+            if (++i >= niter) break;
         }
     }
 }
@@ -456,17 +538,24 @@ cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, ui
 }
 
 template <int S>
+struct TbKernel {
+    static constexpr RfaTbShape sh = RFA_TB_SHAPE[S];
+    using C = TbCfg<S, sh.tx, sh.ty, sh.ry>;
+    static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb>; }
+};
+
+template <int S>
 static cudaError_t launch_blocked_s(const RfaTbParams &p, int grid, cudaStream_t st)
 {
-    using C = TbCfg<S, RFA_TB_TX, RFA_TB_TY, RFA_TB_RY>;
-    auto kern = rfa_blocked_kernel<S, RFA_TB_TX, RFA_TB_TY, RFA_TB_RY>;
+    using K = TbKernel<S>;
+    auto kern = K::get();
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::C::SMEM);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    kern<<<grid, C::NT, C::SMEM, st>>>(p);
+    kern<<<grid, K::C::NT, K::C::SMEM, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -504,13 +593,13 @@ cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const fl
 template <int S>
 static int resident_s()
 {
-    using C = TbCfg<S, RFA_TB_TX, RFA_TB_TY, RFA_TB_RY>;
-    auto kern = rfa_blocked_kernel<S, RFA_TB_TX, RFA_TB_TY, RFA_TB_RY>;
+    using K = TbKernel<S>;
+    auto kern = K::get();
     int dev = 0, sms = 0, occ = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, C::NT, C::SMEM) != cudaSuccess) return 0;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::C::SMEM) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, K::C::NT, K::C::SMEM) != cudaSuccess) return 0;
     return sms * occ;
 }
 

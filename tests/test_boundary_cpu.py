@@ -109,7 +109,8 @@ def test_blocked_plan_covers_the_grid(lib, dims, batch, fused):
     p = binding.plan_query(dims, batch, fused, 148)
     assert p["ok"] == 1
     nx, ny, nz = dims
-    BX, BY = 64, 64
+    BX, BY = p["bx"], p["by"]
+    assert BX % 4 == 0 and BY > 2 * fused
     last_x0 = (p["tiles_x"] - 1) * (BX - 8)
     assert last_x0 + BX >= nx and (p["tiles_x"] == 1 or last_x0 + 4 < nx)
     assert p["tiles_y"] * (BY - 2 * fused) >= ny > (p["tiles_y"] - 1) * (BY - 2 * fused)
