@@ -47,6 +47,7 @@ struct rfa_sim {
     unsigned char *ws = nullptr;         // device workspace
     bool own_ws = false;
     float *theta[2]{};                   // ping-pong temperature images (theta = T - T_a)
+    unsigned char *resid[2]{};           // ping-pong fp16 residual images (rfa_device.cuh: rfa_advance)
     int cur = 0;                         // index of the current image
     uint8_t *state = nullptr;            // packed state bytes
     float *tables = nullptr;             // batch x 3 x 128 coefficients
@@ -65,7 +66,7 @@ struct rfa_sim {
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t theta0, theta1, state, tables, scratch, counters, total;
+    size_t theta0, theta1, resid0, resid1, state, tables, scratch, counters, total;
 };
 
 static bool ws_layout(const int dims[3], int batch, WsLayout &L)
@@ -81,6 +82,10 @@ static bool ws_layout(const int dims[3], int batch, WsLayout &L)
     off = align256(off + nvox * batch * 4);
     L.theta1 = off;
     off = align256(off + nvox * batch * 4);
+    L.resid0 = off;
+    off = align256(off + nvox * batch * 2);
+    L.resid1 = off;
+    off = align256(off + nvox * batch * 2);
     L.state = off;
     off = align256(off + nvox * batch);
     L.tables = off;
@@ -342,6 +347,8 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     }
     s->theta[0] = (float *)(s->ws + L.theta0);
     s->theta[1] = (float *)(s->ws + L.theta1);
+    s->resid[0] = s->ws + L.resid0;
+    s->resid[1] = s->ws + L.resid1;
     s->state = s->ws + L.state;
     s->tables = (float *)(s->ws + L.tables);
     s->scratch = s->ws + L.scratch;
@@ -354,7 +361,7 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
         if (e != cudaSuccess) { rc = cuda_fail(e, "label upload"); break; }
         float theta0[32];
         for (int l = 0; l < 32; ++l) theta0[l] = l < n_tissue ? (float)((double)table[l].t_init - (double)t_blood_c) : 0.f;
-        e = rfa_launch_init(s->g, s->scratch, theta0, s->theta[0], s->state, s->stream);
+        e = rfa_launch_init(s->g, s->scratch, theta0, s->theta[0], s->resid[0], s->state, s->stream);
         s->launches++;
         if (e != cudaSuccess) { rc = cuda_fail(e, "init kernel"); break; }
         for (int b = 0; b < batch && rc == RFA_OK; ++b) rc = upload_table(s, b);
@@ -404,7 +411,7 @@ extern "C" int rfa_set_needle(rfa_sim *s, int scenario, const float tip_mm[3], c
         }
     }
     const float theta_value = (float)((double)value - s->t_blood);
-    e = rfa_launch_needle(s->g, scenario, mdev, mode, theta_value, s->theta[s->cur], s->state, s->stream);
+    e = rfa_launch_needle(s->g, scenario, mdev, mode, theta_value, s->theta[s->cur], s->resid[s->cur], s->state, s->stream);
     s->launches++;
     if (e != cudaSuccess) return cuda_fail(e, "needle kernel");
     s->q_power[scenario] = (mode == RFA_SRC_POWER) ? (double)value : 0.0;
@@ -430,7 +437,7 @@ extern "C" int rfa_set_temperature(rfa_sim *s, int scenario, const float *t_c)
         if (e != cudaSuccess) return cuda_fail(e, "temperature upload");
         src = (const float *)s->scratch;
     }
-    e = rfa_launch_set_temperature(s->g, scenario, src, s->theta[s->cur], s->state, s->stream);
+    e = rfa_launch_set_temperature(s->g, scenario, src, s->theta[s->cur], s->resid[s->cur], s->state, s->stream);
     s->launches++;
     if (e != cudaSuccess) return cuda_fail(e, "set_temperature kernel");
     if (!dev) {
@@ -475,11 +482,11 @@ extern "C" int rfa_step(rfa_sim *s, int n)
             did = std::min(n, s->fused);
             while (did > 1 && !s->plans[did].ok) --did;
             if (s->plans[did].ok)
-                e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->state, s->tables, s->stream);
+                e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
             else
-                e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->state, s->tables, s->stream);
+                e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
         } else {
-            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->state, s->tables, s->stream);
+            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
         }
         s->launches++;
         if (e != cudaSuccess) return cuda_fail(e, "step kernel");

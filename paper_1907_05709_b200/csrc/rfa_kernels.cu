@@ -4,9 +4,11 @@
 //   rfa_blocked_kernel   the hot path: 2.5D z-sweep, S fused time steps per launch
 //   + small set-up / read-back kernels (init, needle, set/get temperature, necrosis, count)
 //
-// Every stepping kernel evaluates rfa_update() (rfa_device.cuh) with the same operands in the same
-// order, so all variants produce bit-identical fields.
+// Every stepping kernel evaluates rfa_bracket() + rfa_advance() (rfa_device.cuh) with the same operands
+// in the same order, so all variants produce bit-identical fields.
 #include <cstdio>
+
+#include <cuda_fp16.h>
 
 #include "rfa_internal.h"
 
@@ -50,7 +52,7 @@ struct Theta0 {
 // label -> initial temperature image: theta = t_init[label] - T_a, state = label id,
 // necrosis on the initial state (R-14).  One launch covers all scenarios.
 __global__ void rfa_init_kernel(size_t nvox, int batch, const uint8_t *__restrict__ labels, Theta0 t0, float thr,
-                                float *__restrict__ theta, uint8_t *__restrict__ state)
+                                float *__restrict__ theta, __half *__restrict__ resid, uint8_t *__restrict__ state)
 {
     size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= nvox) return;
@@ -59,13 +61,15 @@ __global__ void rfa_init_kernel(size_t nvox, int batch, const uint8_t *__restric
     unsigned st = l | (t >= thr ? RFA_ST_NECRO : 0u);
     for (int b = 0; b < batch; ++b) {
         theta[(size_t)b * nvox + v] = t;
+        resid[(size_t)b * nvox + v] = __float2half_rn(0.f);
         state[(size_t)b * nvox + v] = (uint8_t)st;
     }
 }
 
 // needle placement for one scenario (R-15, R-16, R-17)
 __global__ void rfa_needle_kernel(size_t nvox, const uint8_t *__restrict__ mask, int mode, float theta_value,
-                                  float thr, float *__restrict__ theta, uint8_t *__restrict__ state)
+                                  float thr, float *__restrict__ theta, __half *__restrict__ resid,
+                                  uint8_t *__restrict__ state)
 {
     size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= nvox) return;
@@ -74,6 +78,7 @@ __global__ void rfa_needle_kernel(size_t nvox, const uint8_t *__restrict__ mask,
         if (mode == 1) {
             st |= RFA_ST_DIRICHLET;
             theta[v] = theta_value;
+            resid[v] = __float2half_rn(0.f);
             if (theta_value >= thr) st |= RFA_ST_NECRO;
         } else {
             st |= RFA_ST_POWER;
@@ -83,12 +88,14 @@ __global__ void rfa_needle_kernel(size_t nvox, const uint8_t *__restrict__ mask,
 }
 
 __global__ void rfa_set_temperature_kernel(size_t nvox, const float *__restrict__ t_c, float t_blood, float thr,
-                                           float *__restrict__ theta, uint8_t *__restrict__ state)
+                                           float *__restrict__ theta, __half *__restrict__ resid,
+                                           uint8_t *__restrict__ state)
 {
     size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= nvox) return;
     float t = __fsub_rn(t_c[v], t_blood);
     theta[v] = t;
+    resid[v] = __float2half_rn(0.f);
     if (t >= thr) state[v] |= RFA_ST_NECRO;
 }
 
@@ -131,6 +138,7 @@ __global__ void rfa_count_kernel(size_t nvox, const uint8_t *__restrict__ state,
 // plain kernel: Alg. 1 literally -- "for all voxel", one thread each
 // ------------------------------------------------------------------------------------------------
 __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float *__restrict__ tout,
+                                 const __half *__restrict__ rin, __half *__restrict__ rout,
                                  uint8_t *__restrict__ state, const float *__restrict__ tables)
 {
     const size_t nvox = (size_t)g.nx * g.ny * g.nz;
@@ -153,9 +161,12 @@ __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float
     const float zp = k < g.nz - 1 ? T[v + sz] : t;
     const unsigned st = state[gid];
     const unsigned e = st & RFA_ST_INDEX;
-    const float r = rfa_update(t, xm, xp, ym, yp, zm, zp, __ldg(tab + e), __ldg(tab + RFA_TABLE_N + e),
-                               __ldg(tab + 2 * RFA_TABLE_N + e), g.wx, g.wy, g.wz);
+    const float br = rfa_bracket(t, xm, xp, ym, yp, zm, zp, __ldg(tab + RFA_TABLE_N + e),
+                                 __ldg(tab + 2 * RFA_TABLE_N + e), g.wx, g.wy, g.wz);
+    float r, res;
+    rfa_advance(t, __half2float(rin[gid]), __ldg(tab + e), br, r, res);
     tout[gid] = r;
+    rout[gid] = __float2half_rn(res);
     if (r >= g.thr && !(st & RFA_ST_NECRO)) state[gid] = (uint8_t)(st | RFA_ST_NECRO);
 }
 
@@ -172,11 +183,15 @@ __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float
 // x neighbours come from warp shuffles, y neighbours across threads from a double-buffered shared
 // exchange of each thread's first/last row -> one __syncthreads per plane.
 //
-// Arithmetic: the same rounding sequence as rfa_update(), evaluated two voxels at a time with the
-// packed fp32 instructions of sm_100 (add.rn.f32x2 / fma.rn.f32x2 -> FADD2 / FFMA2), so the result is
-// bit-identical to the plain kernel.  Coefficients: when all RY*4 voxels of every thread of the warp
-// carry one label (the common case away from tissue interfaces) they are fetched once per thread and
-// level; otherwise once per voxel.
+// Two code paths per (warp, level), chosen by one warp vote:
+//   FAST  every voxel of every thread of the warp is cold (|theta| < RFA_COMP_MIN, so its residual is
+//         zero by definition) and carries one label per thread: coefficients are fetched once per
+//         thread, the arithmetic runs two voxels per instruction (add.rn.f32x2 / fma.rn.f32x2 ->
+//         FADD2 / FFMA2) in exactly the rounding sequence of rfa_bracket()/rfa_advance() with r = 0.
+//   SLOW  anything else (near the needle, tissue interfaces): rfa_bracket()/rfa_advance() per voxel,
+//         residuals read from the fp16 residual image (level 0) or passed between levels through
+//         shared memory.
+// Both give bit-identical results to the plain kernel.
 //
 // Halos: x tiles overlap by 8 columns (4 = one float4 per side, S <= 4), y tiles and z chunks carry
 // S halo rows / planes per side.  At the outer y and z faces the halo is loaded MIRRORED
@@ -186,6 +201,8 @@ __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float
 struct RfaTbParams {
     const float *tin;
     float *tout;
+    const __half *rin;
+    __half *rout;
     uint8_t *state;
     const float *tables;
     int nx, ny, nz, batch;
@@ -194,19 +211,23 @@ struct RfaTbParams {
     int tiles_x, tiles_y, nzc, zchunk, n_items;
 };
 
+constexpr int rfa_pow2_at_least(int n) { return n <= 1 ? 1 : 2 * rfa_pow2_at_least((n + 1) / 2); }
+
 template <int S, int TX, int TY, int RY>
 struct TbCfg {
     static constexpr int NT = TX * TY;
     static constexpr int BX = 4 * TX;
     static constexpr int BY = RY * TY;
-    static constexpr int PD = 1;              // prefetch distance (planes in flight)
-    static constexpr int DT = PD + 1;         // temperature ring depth
-    static constexpr int DS = PD + S + 1;     // state ring depth (level k reads plane i-k-1)
+    static constexpr int PD = 1;                                  // prefetch distance (planes in flight)
+    static constexpr int DT = 2;                                  // temperature ring depth (PD + 1)
+    static constexpr int DS = rfa_pow2_at_least(PD + S + 1);      // state ring depth (level k reads plane i-k-1)
+    static constexpr int NR = S > 1 ? S - 1 : 1;                  // inter-level residual buffers
     static constexpr size_t RING_T = (size_t)DT * RY * NT * 16;
     static constexpr size_t EXCH = (size_t)S * 2 * 2 * NT * 16;
     static constexpr size_t RING_S = (size_t)DS * RY * NT * 4;
+    static constexpr size_t RSM = (size_t)NR * 2 * RY * NT * 8;
     static constexpr size_t TAB = 3 * RFA_TABLE_N * 4;
-    static constexpr size_t SMEM = RING_T + EXCH + RING_S + TAB;
+    static constexpr size_t SMEM = RING_T + EXCH + RING_S + RSM + TAB;
 };
 
 typedef unsigned long long u64;
@@ -229,6 +250,22 @@ __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
     return r;
 }
+__device__ __forceinline__ float max3abs(float a, float b, float c) { return fmaxf(fmaxf(fabsf(a), fabsf(b)), fabsf(c)); }
+__device__ __forceinline__ float max_abs4(const float4 v, float m) { return fmaxf(max3abs(v.x, v.y, v.z), fmaxf(fabsf(v.w), m)); }
+__device__ __forceinline__ uint2 pack_h4(float a, float b, float c, float d)
+{
+    const __half2 lo = __floats2half2_rn(a, b), hi = __floats2half2_rn(c, d);
+    uint2 r;
+    r.x = *reinterpret_cast<const unsigned *>(&lo);
+    r.y = *reinterpret_cast<const unsigned *>(&hi);
+    return r;
+}
+__device__ __forceinline__ float4 unpack_h4(const uint2 v)
+{
+    const float2 lo = __half22float2(*reinterpret_cast<const __half2 *>(&v.x));
+    const float2 hi = __half22float2(*reinterpret_cast<const __half2 *>(&v.y));
+    return make_float4(lo.x, lo.y, hi.x, hi.y);
+}
 
 template <int I>
 struct IC {
@@ -242,10 +279,11 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
     constexpr int NT = C::NT, BX = C::BX, BY = C::BY, PD = C::PD, DT = C::DT, DS = C::DS;
     static_assert(RY == 4 || RY == 2, "state words of a thread are read as one vector");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4 *ringT = reinterpret_cast<float4 *>(smem_raw);                  // [DT][RY][NT]
-    float4 *exch = reinterpret_cast<float4 *>(smem_raw + C::RING_T);       // [S][2 parity][2 top/bot][NT]
-    uint32_t *ringS = reinterpret_cast<uint32_t *>(smem_raw + C::RING_T + C::EXCH);   // [DS][NT][RY]
-    float *tab = reinterpret_cast<float *>(smem_raw + C::RING_T + C::EXCH + C::RING_S);   // [3][128]
+    float4 *ringT = reinterpret_cast<float4 *>(smem_raw);                                          // [DT][RY][NT]
+    float4 *exch = reinterpret_cast<float4 *>(smem_raw + C::RING_T);                               // [S][2 parity][2 top/bot][NT]
+    uint32_t *ringS = reinterpret_cast<uint32_t *>(smem_raw + C::RING_T + C::EXCH);                // [DS][NT][RY]
+    uint2 *rsm = reinterpret_cast<uint2 *>(smem_raw + C::RING_T + C::EXCH + C::RING_S);            // [NR][2 parity][RY][NT]
+    float *tab = reinterpret_cast<float *>(smem_raw + C::RING_T + C::EXCH + C::RING_S + C::RSM);   // [3][128]
 
     const int tid = threadIdx.x;
     const int tx = tid % TX, ty = tid / TX;
@@ -254,9 +292,11 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
 
     for (int e = tid; e < S * 2 * 2 * NT; e += NT) exch[e] = make_float4(0.f, 0.f, 0.f, 0.f);
 
-    const size_t plane4 = (size_t)P.ny * P.nx4;       // float4 (= state words) per plane
-    const u64 wx2 = pk(P.wx, P.wx), wy2 = pk(P.wy, P.wy), wz2 = pk(P.wz, P.wz), m2 = pk(-2.0f, -2.0f);
+    const unsigned plane4 = (unsigned)(P.ny * P.nx4);       // float4 (= state words = residual quads) per plane
+    const float wx = P.wx, wy = P.wy, wz = P.wz;
+    const u64 wx2 = pk(wx, wx), wy2 = pk(wy, wy), wz2 = pk(wz, wz), m2 = pk(-2.0f, -2.0f), zero2 = pk(0.f, 0.f);
     const float thr = P.thr;
+    const float thr_filter = fmaxf(thr, 0.0f);               // max|theta'| below this: no voxel can reach thr
     int cur_b = -1;
 
     for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
@@ -290,6 +330,8 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
         const size_t base4 = (size_t)b * P.nz * plane4;
         const float4 *tin4 = reinterpret_cast<const float4 *>(P.tin) + base4;
         float4 *tout4 = reinterpret_cast<float4 *>(P.tout) + base4;
+        const uint2 *rin2 = reinterpret_cast<const uint2 *>(P.rin) + base4;
+        uint2 *rout2 = reinterpret_cast<uint2 *>(P.rout) + base4;
         uint32_t *st4 = reinterpret_cast<uint32_t *>(P.state) + base4;
 
         __syncthreads();                                   // previous item done with tab / exchange
@@ -298,27 +340,31 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
             cur_b = b;
         }
 
-        // q[k][slot][r]: three planes of level k (see the header comment); nbq: their necrosis bits
+        // q[k][slot][r]: three planes of level k (see the header comment); per plane: nbq = necrosis bits set
+        // on the way up, hotq = some voxel of this thread has |theta| >= RFA_COMP_MIN, rvq = its residual
+        // sits in rsm (levels >= 1; level 0 residuals live in the HBM residual image)
         float4 q[S][3][RY];
         unsigned nbq[S][3];
+        bool hotq[S][3], rvq[S][3];
 #pragma unroll
         for (int k = 0; k < S; ++k)
 #pragma unroll
             for (int s = 0; s < 3; ++s) {
                 nbq[k][s] = 0;
+                hotq[k][s] = false;
+                rvq[k][s] = false;
 #pragma unroll
                 for (int r = 0; r < RY; ++r) q[k][s][r] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
 
         const int niter = (z1 - z0) + 2 * S;
         auto issue = [&](int j) {
-            const int zs = rfa_reflect(z0 - S + j, P.nz);
-            const size_t pl = (size_t)zs * plane4;
-            const int sT = j % DT, sS = j % DS;
+            const unsigned pl = (unsigned)rfa_reflect(z0 - S + j, P.nz) * plane4;
+            const int sT = j & (DT - 1), sS = j & (DS - 1);
 #pragma unroll
             for (int r = 0; r < RY; ++r) {
-                cp_async16(&ringT[(sT * RY + r) * NT + tid], tin4 + pl + row_src[r]);
-                cp_async4(&ringS[(sS * NT + tid) * RY + r], st4 + pl + row_src[r]);
+                cp_async16(&ringT[(sT * RY + r) * NT + tid], tin4 + (pl + row_src[r]));
+                cp_async4(&ringS[(sS * NT + tid) * RY + r], st4 + (pl + row_src[r]));
             }
         };
 #pragma unroll
@@ -336,14 +382,20 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
             cp_async_commit();
             cp_async_wait<PD>();
             {
-                const int sT = i % DT;
+                const int sT = i & (DT - 1);
+                float m = 0.f;
 #pragma unroll
-                for (int r = 0; r < RY; ++r) q[0][PH][r] = ringT[(sT * RY + r) * NT + tid];
+                for (int r = 0; r < RY; ++r) {
+                    q[0][PH][r] = ringT[(sT * RY + r) * NT + tid];
+                    m = max_abs4(q[0][PH][r], m);
+                }
                 nbq[0][PH] = 0;
+                hotq[0][PH] = m >= RFA_COMP_MIN;
             }
             __syncthreads();                               // exchange rows of iteration i-1 are visible
             const int par_w = i & 1, par_r = par_w ^ 1;
             float4 out[RY];
+            uint2 rout[RY];
             unsigned nb_out = 0;
 #pragma unroll
             for (int k = 0; k < S; ++k) {
@@ -352,8 +404,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 exch[((k * 2 + par_w) * 2 + 1) * NT + tid] = q[k][PH][RY - 1];
                 const float4 above = exch[((k * 2 + par_r) * 2 + 1) * NT + up_tid];
                 const float4 below = exch[((k * 2 + par_r) * 2 + 0) * NT + dn_tid];
-                int sS = i % DS - (k + 1);                  // state of the centre plane
-                if (sS < 0) sS += DS;
+                const int sS = (i - (k + 1)) & (DS - 1);    // state of the centre plane
                 uint32_t sw[RY];
                 if constexpr (RY == 4) {
                     const uint4 v = *reinterpret_cast<const uint4 *>(&ringS[(sS * NT + tid) * RY]);
@@ -362,81 +413,105 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                     const uint2 v = *reinterpret_cast<const uint2 *>(&ringS[(sS * NT + tid) * RY]);
                     sw[0] = v.x; sw[1] = v.y;
                 }
-                // one label for all voxels of every thread of the warp?
+                // one label for all voxels of this thread?
                 uint32_t diff = sw[0] ^ __byte_perm(sw[0], 0, 0);
 #pragma unroll
                 for (int r = 1; r < RY; ++r) diff |= sw[0] ^ sw[r];
-                const bool uni = __all_sync(0xffffffffu, (diff & 0x7f7f7f7fu) == 0u);
-                u64 a01, a23, n01, n23, q01, q23;
-                if (uni) {
+                const bool fast = __all_sync(0xffffffffu, (diff & 0x7f7f7f7fu) == 0u && !hotq[k][CE]);
+                float mx = 0.f;                            // max |theta'| over this thread's voxels
+                float4 o[RY];
+                if (fast) {
                     const unsigned e = sw[0] & RFA_ST_INDEX;
                     const float a = tab[e], nk = tab[RFA_TABLE_N + e], qa = tab[2 * RFA_TABLE_N + e];
-                    a01 = a23 = pk(a, a);
-                    n01 = n23 = pk(nk, nk);
-                    q01 = q23 = pk(qa, qa);
-                }
-                float mx = -3.0e38f;
-#pragma unroll
-                for (int r = 0; r < RY; ++r) {
-                    const float4 c = q[k][CE][r];
-                    const float4 u = (r == 0) ? above : q[k][CE][r - 1];
-                    const float4 d = (r == RY - 1) ? below : q[k][CE][r + 1];
-                    float left = __shfl_up_sync(0xffffffffu, c.w, 1, TX);
-                    float right = __shfl_down_sync(0xffffffffu, c.x, 1, TX);
-                    if (xl_self) left = c.x;               // zero flux at the outer x faces (R-7)
-                    if (xr_self) right = c.w;
-                    if (!uni) {
-                        const uint32_t w = sw[r];
-                        const unsigned e0 = w & RFA_ST_INDEX, e1 = (w >> 8) & RFA_ST_INDEX,
-                                       e2 = (w >> 16) & RFA_ST_INDEX, e3 = (w >> 24) & RFA_ST_INDEX;
-                        a01 = pk(tab[e0], tab[e1]);
-                        a23 = pk(tab[e2], tab[e3]);
-                        n01 = pk(tab[RFA_TABLE_N + e0], tab[RFA_TABLE_N + e1]);
-                        n23 = pk(tab[RFA_TABLE_N + e2], tab[RFA_TABLE_N + e3]);
-                        q01 = pk(tab[2 * RFA_TABLE_N + e0], tab[2 * RFA_TABLE_N + e1]);
-                        q23 = pk(tab[2 * RFA_TABLE_N + e2], tab[2 * RFA_TABLE_N + e3]);
-                    }
-                    const float4 zm = q[k][MI][r], zp = q[k][PH][r];
-                    // same rounding sequence as rfa_update(), two voxels per instruction
-                    const u64 t01 = pk(c.x, c.y), t23 = pk(c.z, c.w);
-                    const u64 sx01 = pk(__fadd_rn(left, c.y), __fadd_rn(c.x, c.z));
-                    const u64 sx23 = pk(__fadd_rn(c.y, c.w), __fadd_rn(c.z, right));
-                    const u64 sy01 = add2(pk(u.x, u.y), pk(d.x, d.y)), sy23 = add2(pk(u.z, u.w), pk(d.z, d.w));
-                    const u64 sz01 = add2(pk(zm.x, zm.y), pk(zp.x, zp.y)), sz23 = add2(pk(zm.z, zm.w), pk(zp.z, zp.w));
-                    const u64 l01 = fma2(wz2, sz01, fma2(wy2, sy01, fma2(wx2, sx01, fma2(n01, t01, q01))));
-                    const u64 l23 = fma2(wz2, sz23, fma2(wy2, sy23, fma2(wx2, sx23, fma2(n23, t23, q23))));
-                    const u64 o01 = fma2(a01, fma2(m2, t01, l01), t01);
-                    const u64 o23 = fma2(a23, fma2(m2, t23, l23), t23);
-                    float4 o;
-                    upk(o01, o.x, o.y);
-                    upk(o23, o.z, o.w);
-                    mx = fmaxf(mx, fmaxf(fmaxf(o.x, o.y), fmaxf(o.z, o.w)));
-                    if (k + 1 < S) q[(k + 1) % S][PH][r] = o;
-                    else out[r] = o;
-                }
-                unsigned nb_o = nbq[k][CE];
-                if (mx >= thr) {                           // rare: some voxel of this thread reached 60 C
+                    const u64 a2 = pk(a, a), n2 = pk(nk, nk), q2 = pk(qa, qa);
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
-                        const float4 o = (k + 1 < S) ? q[(k + 1) % S][PH][r] : out[r];
-                        nb_o |= (o.x >= thr ? 1u : 0u) << (4 * r);
-                        nb_o |= (o.y >= thr ? 2u : 0u) << (4 * r);
-                        nb_o |= (o.z >= thr ? 4u : 0u) << (4 * r);
-                        nb_o |= (o.w >= thr ? 8u : 0u) << (4 * r);
+                        const float4 c = q[k][CE][r];
+                        const float4 u = (r == 0) ? above : q[k][CE][r - 1];
+                        const float4 d = (r == RY - 1) ? below : q[k][CE][r + 1];
+                        float left = __shfl_up_sync(0xffffffffu, c.w, 1, TX);
+                        float right = __shfl_down_sync(0xffffffffu, c.x, 1, TX);
+                        if (xl_self) left = c.x;           // zero flux at the outer x faces (R-7)
+                        if (xr_self) right = c.w;
+                        const float4 zm = q[k][MI][r], zp = q[k][PH][r];
+                        // rfa_bracket() + rfa_advance() with r = 0, two voxels per instruction
+                        const u64 t01 = pk(c.x, c.y), t23 = pk(c.z, c.w);
+                        const u64 sx01 = pk(__fadd_rn(left, c.y), __fadd_rn(c.x, c.z));
+                        const u64 sx23 = pk(__fadd_rn(c.y, c.w), __fadd_rn(c.z, right));
+                        const u64 sy01 = add2(pk(u.x, u.y), pk(d.x, d.y)), sy23 = add2(pk(u.z, u.w), pk(d.z, d.w));
+                        const u64 sz01 = add2(pk(zm.x, zm.y), pk(zp.x, zp.y)), sz23 = add2(pk(zm.z, zm.w), pk(zp.z, zp.w));
+                        const u64 l01 = fma2(wz2, sz01, fma2(wy2, sy01, fma2(wx2, sx01, fma2(n2, t01, q2))));
+                        const u64 l23 = fma2(wz2, sz23, fma2(wy2, sy23, fma2(wx2, sx23, fma2(n2, t23, q2))));
+                        const u64 o01 = add2(t01, fma2(a2, fma2(m2, t01, l01), zero2));
+                        const u64 o23 = add2(t23, fma2(a2, fma2(m2, t23, l23), zero2));
+                        upk(o01, o[r].x, o[r].y);
+                        upk(o23, o[r].z, o[r].w);
+                        mx = max_abs4(o[r], mx);
+                        if (k + 1 == S) rout[r] = make_uint2(0u, 0u);
+                    }
+                    if (k + 1 < S) rvq[k + 1][PH] = false;
+                } else {
+                    const unsigned plc = (unsigned)rfa_reflect(z0 - S + i - 1, P.nz) * plane4;   // level-0 centre plane
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        const float4 c = q[k][CE][r];
+                        const float4 u = (r == 0) ? above : q[k][CE][r - 1];
+                        const float4 d = (r == RY - 1) ? below : q[k][CE][r + 1];
+                        float left = __shfl_up_sync(0xffffffffu, c.w, 1, TX);
+                        float right = __shfl_down_sync(0xffffffffu, c.x, 1, TX);
+                        if (xl_self) left = c.x;
+                        if (xr_self) right = c.w;
+                        const float4 zm = q[k][MI][r], zp = q[k][PH][r];
+                        float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (hotq[k][CE]) {
+                            if (k == 0) ri = unpack_h4(__ldg(rin2 + (plc + row_src[r])));
+                            else if (rvq[k][CE]) ri = unpack_h4(rsm[(((k - 1) * 2 + par_r) * RY + r) * NT + tid]);
+                        }
+                        const uint32_t w = sw[r];
+                        const unsigned e0 = w & RFA_ST_INDEX, e1 = (w >> 8) & RFA_ST_INDEX, e2 = (w >> 16) & RFA_ST_INDEX,
+                                       e3 = (w >> 24) & RFA_ST_INDEX;
+                        float4 ro;
+                        rfa_advance(c.x, ri.x, tab[e0], rfa_bracket(c.x, left, c.y, u.x, d.x, zm.x, zp.x, tab[RFA_TABLE_N + e0], tab[2 * RFA_TABLE_N + e0], wx, wy, wz), o[r].x, ro.x);
+                        rfa_advance(c.y, ri.y, tab[e1], rfa_bracket(c.y, c.x, c.z, u.y, d.y, zm.y, zp.y, tab[RFA_TABLE_N + e1], tab[2 * RFA_TABLE_N + e1], wx, wy, wz), o[r].y, ro.y);
+                        rfa_advance(c.z, ri.z, tab[e2], rfa_bracket(c.z, c.y, c.w, u.z, d.z, zm.z, zp.z, tab[RFA_TABLE_N + e2], tab[2 * RFA_TABLE_N + e2], wx, wy, wz), o[r].z, ro.z);
+                        rfa_advance(c.w, ri.w, tab[e3], rfa_bracket(c.w, c.z, right, u.w, d.w, zm.w, zp.w, tab[RFA_TABLE_N + e3], tab[2 * RFA_TABLE_N + e3], wx, wy, wz), o[r].w, ro.w);
+                        mx = max_abs4(o[r], mx);
+                        const uint2 rp = pack_h4(ro.x, ro.y, ro.z, ro.w);
+                        if (k + 1 < S) rsm[((k * 2 + par_w) * RY + r) * NT + tid] = rp;
+                        else rout[r] = rp;
+                    }
+                    if (k + 1 < S) rvq[k + 1][PH] = true;
+                }
+                unsigned nb_o = nbq[k][CE];
+                if (mx >= thr_filter) {                    // rare: some voxel of this thread may have reached 60 C
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        nb_o |= (o[r].x >= thr ? 1u : 0u) << (4 * r);
+                        nb_o |= (o[r].y >= thr ? 2u : 0u) << (4 * r);
+                        nb_o |= (o[r].z >= thr ? 4u : 0u) << (4 * r);
+                        nb_o |= (o[r].w >= thr ? 8u : 0u) << (4 * r);
                     }
                 }
-                if (k + 1 < S) nbq[(k + 1) % S][PH] = nb_o;
-                else nb_out = nb_o;
+                if (k + 1 < S) {
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) q[(k + 1) % S][PH][r] = o[r];
+                    nbq[(k + 1) % S][PH] = nb_o;
+                    hotq[(k + 1) % S][PH] = mx >= RFA_COMP_MIN;
+                } else {
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) out[r] = o[r];
+                    nb_out = nb_o;
+                }
             }
             // `out` is level S of plane z0 + (i - 2S)
             if (i >= 2 * S) {
-                const size_t pl = (size_t)(z0 + i - 2 * S) * plane4;
-                int sS = i % DS - S;
-                if (sS < 0) sS += DS;
+                const unsigned pl = (unsigned)(z0 + i - 2 * S) * plane4;
+                const int sS = (i - S) & (DS - 1);
 #pragma unroll
                 for (int r = 0; r < RY; ++r) {
                     if (row_ok & (1u << r)) {
                         tout4[pl + row_dst[r]] = out[r];
+                        rout2[pl + row_dst[r]] = rout[r];
                         const unsigned bits = (nb_out >> (4 * r)) & 0xfu;
                         if (bits) {
                             const uint32_t w = ringS[(sS * NT + tid) * RY + r];
@@ -472,31 +547,33 @@ cudaError_t rfa_launch_table(const RfaTableHost &tbl, float *dst, cudaStream_t s
 }
 
 cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const float *theta0_by_label, float *theta,
-                            uint8_t *state, cudaStream_t st)
+                            void *resid, uint8_t *state, cudaStream_t st)
 {
     Theta0 t0;
     for (int i = 0; i < 32; ++i) t0.v[i] = theta0_by_label[i];
     size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    rfa_init_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(nvox, g.batch, labels_dev, t0, g.thr, theta, state);
+    rfa_init_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(nvox, g.batch, labels_dev, t0, g.thr, theta, (__half *)resid, state);
     return cudaGetLastError();
 }
 
 cudaError_t rfa_launch_needle(const RfaGrid &g, int scenario, const uint8_t *mask_dev, int mode, float theta_value,
-                              float *theta, uint8_t *state, cudaStream_t st)
+                              float *theta, void *resid, uint8_t *state, cudaStream_t st)
 {
     size_t nvox = (size_t)g.nx * g.ny * g.nz;
     rfa_needle_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(nvox, mask_dev, mode, theta_value, g.thr,
                                                              theta + (size_t)scenario * nvox,
+                                                             (__half *)resid + (size_t)scenario * nvox,
                                                              state + (size_t)scenario * nvox);
     return cudaGetLastError();
 }
 
 cudaError_t rfa_launch_set_temperature(const RfaGrid &g, int scenario, const float *t_dev, float *theta,
-                                       uint8_t *state, cudaStream_t st)
+                                       void *resid, uint8_t *state, cudaStream_t st)
 {
     size_t nvox = (size_t)g.nx * g.ny * g.nz;
     rfa_set_temperature_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(nvox, t_dev, g.t_blood, g.thr,
                                                                       theta + (size_t)scenario * nvox,
+                                                                      (__half *)resid + (size_t)scenario * nvox,
                                                                       state + (size_t)scenario * nvox);
     return cudaGetLastError();
 }
@@ -529,11 +606,11 @@ cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *stat
     return cudaGetLastError();
 }
 
-cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, uint8_t *state, const float *tables,
-                             cudaStream_t st)
+cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, const void *rin, void *rout,
+                             uint8_t *state, const float *tables, cudaStream_t st)
 {
     size_t n = (size_t)g.nx * g.ny * g.nz * g.batch;
-    rfa_plain_kernel<<<blocks_for(n, 256), 256, 0, st>>>(g, tin, tout, state, tables);
+    rfa_plain_kernel<<<blocks_for(n, 256), 256, 0, st>>>(g, tin, tout, (const __half *)rin, (__half *)rout, state, tables);
     return cudaGetLastError();
 }
 
@@ -560,11 +637,13 @@ static cudaError_t launch_blocked_s(const RfaTbParams &p, int grid, cudaStream_t
 }
 
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
-                               uint8_t *state, const float *tables, cudaStream_t st)
+                               const void *rin, void *rout, uint8_t *state, const float *tables, cudaStream_t st)
 {
     RfaTbParams p;
     p.tin = tin;
     p.tout = tout;
+    p.rin = (const __half *)rin;
+    p.rout = (__half *)rout;
     p.state = state;
     p.tables = tables;
     p.nx = g.nx;
