@@ -183,15 +183,15 @@ __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float
 // x neighbours come from warp shuffles, y neighbours across threads from a double-buffered shared
 // exchange of each thread's first/last row -> one __syncthreads per plane.
 //
-// Two code paths per (warp, level), chosen by one warp vote:
-//   FAST  every voxel of every thread of the warp is cold (|theta| < RFA_COMP_MIN, so its residual is
-//         zero by definition) and carries one label per thread: coefficients are fetched once per
-//         thread, the arithmetic runs two voxels per instruction (add.rn.f32x2 / fma.rn.f32x2 ->
-//         FADD2 / FFMA2) in exactly the rounding sequence of rfa_bracket()/rfa_advance() with r = 0.
-//   SLOW  anything else (near the needle, tissue interfaces): rfa_bracket()/rfa_advance() per voxel,
-//         residuals read from the fp16 residual image (level 0) or passed between levels through
-//         shared memory.
-// Both give bit-identical results to the plain kernel.
+// The arithmetic runs two voxels per instruction (add.rn.f32x2 / fma.rn.f32x2 -> FADD2 / FFMA2) in
+// exactly the rounding sequence of rfa_bracket()/rfa_advance().  Three code paths per (warp, level),
+// chosen by two warp votes taken before the barrier:
+//   cold + one label per thread   every voxel has |theta| < RFA_COMP_MIN (residual zero by definition):
+//                                 coefficients fetched once per thread, theta' = theta + fma(a, g, 0)
+//   cold + mixed labels           tissue interfaces: coefficients gathered per voxel
+//   hot                           near the needle: compensated add in full; residuals come from the
+//                                 fp16 residual image (level 0) or from the level below through shared memory
+// All give bit-identical results to the plain kernel.
 //
 // Halos: x tiles overlap by 8 columns (4 = one float4 per side, S <= 4), y tiles and z chunks carry
 // S halo rows / planes per side.  At the outer y and z faces the halo is loaded MIRRORED
@@ -392,6 +392,26 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 nbq[0][PH] = 0;
                 hotq[0][PH] = m >= RFA_COMP_MIN;
             }
+            // state words of the S centre planes and the two warp votes per level that pick the code path:
+            // thread-private data, so all of it is issued before the barrier and overlaps the wait
+            uint32_t sw[S][RY];
+            bool uni[S], cold[S];
+#pragma unroll
+            for (int k = 0; k < S; ++k) {
+                const int sS = (i - (k + 1)) & (DS - 1);
+                if constexpr (RY == 4) {
+                    const uint4 v = *reinterpret_cast<const uint4 *>(&ringS[(sS * NT + tid) * RY]);
+                    sw[k][0] = v.x; sw[k][1] = v.y; sw[k][2] = v.z; sw[k][3] = v.w;
+                } else {
+                    const uint2 v = *reinterpret_cast<const uint2 *>(&ringS[(sS * NT + tid) * RY]);
+                    sw[k][0] = v.x; sw[k][1] = v.y;
+                }
+                uint32_t diff = sw[k][0] ^ __byte_perm(sw[k][0], 0, 0);
+#pragma unroll
+                for (int r = 1; r < RY; ++r) diff |= sw[k][0] ^ sw[k][r];
+                uni[k] = __all_sync(0xffffffffu, (diff & 0x7f7f7f7fu) == 0u);    // one label per thread
+                cold[k] = __all_sync(0xffffffffu, !hotq[k][CE]);                  // all residuals are zero
+            }
             __syncthreads();                               // exchange rows of iteration i-1 are visible
             const int par_w = i & 1, par_r = par_w ^ 1;
             float4 out[RY];
@@ -404,79 +424,103 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 exch[((k * 2 + par_w) * 2 + 1) * NT + tid] = q[k][PH][RY - 1];
                 const float4 above = exch[((k * 2 + par_r) * 2 + 1) * NT + up_tid];
                 const float4 below = exch[((k * 2 + par_r) * 2 + 0) * NT + dn_tid];
-                const int sS = (i - (k + 1)) & (DS - 1);    // state of the centre plane
-                uint32_t sw[RY];
-                if constexpr (RY == 4) {
-                    const uint4 v = *reinterpret_cast<const uint4 *>(&ringS[(sS * NT + tid) * RY]);
-                    sw[0] = v.x; sw[1] = v.y; sw[2] = v.z; sw[3] = v.w;
-                } else {
-                    const uint2 v = *reinterpret_cast<const uint2 *>(&ringS[(sS * NT + tid) * RY]);
-                    sw[0] = v.x; sw[1] = v.y;
-                }
-                // one label for all voxels of this thread?
-                uint32_t diff = sw[0] ^ __byte_perm(sw[0], 0, 0);
-#pragma unroll
-                for (int r = 1; r < RY; ++r) diff |= sw[0] ^ sw[r];
-                const bool fast = __all_sync(0xffffffffu, (diff & 0x7f7f7f7fu) == 0u && !hotq[k][CE]);
                 float mx = 0.f;                            // max |theta'| over this thread's voxels
                 float4 o[RY];
-                if (fast) {
-                    const unsigned e = sw[0] & RFA_ST_INDEX;
-                    const float a = tab[e], nk = tab[RFA_TABLE_N + e], qa = tab[2 * RFA_TABLE_N + e];
-                    const u64 a2 = pk(a, a), n2 = pk(nk, nk), q2 = pk(qa, qa);
+
+                // g = rfa_bracket() of the four voxels of row r, two voxels per instruction
+                auto bracket_row = [&](const int r, const u64 n01, const u64 n23, const u64 q01, const u64 q23,
+                                       u64 &t01, u64 &t23, u64 &g01, u64 &g23) {
+                    const float4 c = q[k][CE][r];
+                    const float4 u = (r == 0) ? above : q[k][CE][r > 0 ? r - 1 : 0];
+                    const float4 d = (r == RY - 1) ? below : q[k][CE][r < RY - 1 ? r + 1 : r];
+                    float left = __shfl_up_sync(0xffffffffu, c.w, 1, TX);
+                    float right = __shfl_down_sync(0xffffffffu, c.x, 1, TX);
+                    if (xl_self) left = c.x;               // zero flux at the outer x faces (R-7)
+                    if (xr_self) right = c.w;
+                    const float4 zm = q[k][MI][r], zp = q[k][PH][r];
+                    t01 = pk(c.x, c.y);
+                    t23 = pk(c.z, c.w);
+                    const u64 sx01 = pk(__fadd_rn(left, c.y), __fadd_rn(c.x, c.z));
+                    const u64 sx23 = pk(__fadd_rn(c.y, c.w), __fadd_rn(c.z, right));
+                    const u64 sy01 = add2(pk(u.x, u.y), pk(d.x, d.y)), sy23 = add2(pk(u.z, u.w), pk(d.z, d.w));
+                    const u64 sz01 = add2(pk(zm.x, zm.y), pk(zp.x, zp.y)), sz23 = add2(pk(zm.z, zm.w), pk(zp.z, zp.w));
+                    const u64 l01 = fma2(wz2, sz01, fma2(wy2, sy01, fma2(wx2, sx01, fma2(n01, t01, q01))));
+                    const u64 l23 = fma2(wz2, sz23, fma2(wy2, sy23, fma2(wx2, sx23, fma2(n23, t23, q23))));
+                    g01 = fma2(m2, t01, l01);
+                    g23 = fma2(m2, t23, l23);
+                };
+                // per-voxel coefficients of row r (tissue interfaces, needle voxels)
+                auto gather_row = [&](const int r, u64 &a01, u64 &a23, u64 &n01, u64 &n23, u64 &q01, u64 &q23) {
+                    const uint32_t w = sw[k][r];
+                    const unsigned e0 = w & RFA_ST_INDEX, e1 = (w >> 8) & RFA_ST_INDEX, e2 = (w >> 16) & RFA_ST_INDEX,
+                                   e3 = (w >> 24) & RFA_ST_INDEX;
+                    a01 = pk(tab[e0], tab[e1]);
+                    a23 = pk(tab[e2], tab[e3]);
+                    n01 = pk(tab[RFA_TABLE_N + e0], tab[RFA_TABLE_N + e1]);
+                    n23 = pk(tab[RFA_TABLE_N + e2], tab[RFA_TABLE_N + e3]);
+                    q01 = pk(tab[2 * RFA_TABLE_N + e0], tab[2 * RFA_TABLE_N + e1]);
+                    q23 = pk(tab[2 * RFA_TABLE_N + e2], tab[2 * RFA_TABLE_N + e3]);
+                };
+
+                if (cold[k]) {
+                    // rfa_advance() with r = 0:  theta' = theta + fma(a, g, 0)
+                    if (uni[k]) {
+                        const unsigned e = sw[k][0] & RFA_ST_INDEX;
+                        const float a = tab[e], nk = tab[RFA_TABLE_N + e], qa = tab[2 * RFA_TABLE_N + e];
+                        const u64 a2 = pk(a, a), n2 = pk(nk, nk), q2 = pk(qa, qa);
 #pragma unroll
-                    for (int r = 0; r < RY; ++r) {
-                        const float4 c = q[k][CE][r];
-                        const float4 u = (r == 0) ? above : q[k][CE][r - 1];
-                        const float4 d = (r == RY - 1) ? below : q[k][CE][r + 1];
-                        float left = __shfl_up_sync(0xffffffffu, c.w, 1, TX);
-                        float right = __shfl_down_sync(0xffffffffu, c.x, 1, TX);
-                        if (xl_self) left = c.x;           // zero flux at the outer x faces (R-7)
-                        if (xr_self) right = c.w;
-                        const float4 zm = q[k][MI][r], zp = q[k][PH][r];
-                        // rfa_bracket() + rfa_advance() with r = 0, two voxels per instruction
-                        const u64 t01 = pk(c.x, c.y), t23 = pk(c.z, c.w);
-                        const u64 sx01 = pk(__fadd_rn(left, c.y), __fadd_rn(c.x, c.z));
-                        const u64 sx23 = pk(__fadd_rn(c.y, c.w), __fadd_rn(c.z, right));
-                        const u64 sy01 = add2(pk(u.x, u.y), pk(d.x, d.y)), sy23 = add2(pk(u.z, u.w), pk(d.z, d.w));
-                        const u64 sz01 = add2(pk(zm.x, zm.y), pk(zp.x, zp.y)), sz23 = add2(pk(zm.z, zm.w), pk(zp.z, zp.w));
-                        const u64 l01 = fma2(wz2, sz01, fma2(wy2, sy01, fma2(wx2, sx01, fma2(n2, t01, q2))));
-                        const u64 l23 = fma2(wz2, sz23, fma2(wy2, sy23, fma2(wx2, sx23, fma2(n2, t23, q2))));
-                        const u64 o01 = add2(t01, fma2(a2, fma2(m2, t01, l01), zero2));
-                        const u64 o23 = add2(t23, fma2(a2, fma2(m2, t23, l23), zero2));
-                        upk(o01, o[r].x, o[r].y);
-                        upk(o23, o[r].z, o[r].w);
-                        mx = max_abs4(o[r], mx);
-                        if (k + 1 == S) rout[r] = make_uint2(0u, 0u);
+                        for (int r = 0; r < RY; ++r) {
+                            u64 t01, t23, g01, g23;
+                            bracket_row(r, n2, n2, q2, q2, t01, t23, g01, g23);
+                            upk(add2(t01, fma2(a2, g01, zero2)), o[r].x, o[r].y);
+                            upk(add2(t23, fma2(a2, g23, zero2)), o[r].z, o[r].w);
+                            mx = max_abs4(o[r], mx);
+                        }
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < RY; ++r) {
+                            u64 a01, a23, n01, n23, q01, q23, t01, t23, g01, g23;
+                            gather_row(r, a01, a23, n01, n23, q01, q23);
+                            bracket_row(r, n01, n23, q01, q23, t01, t23, g01, g23);
+                            upk(add2(t01, fma2(a01, g01, zero2)), o[r].x, o[r].y);
+                            upk(add2(t23, fma2(a23, g23, zero2)), o[r].z, o[r].w);
+                            mx = max_abs4(o[r], mx);
+                        }
                     }
                     if (k + 1 < S) rvq[k + 1][PH] = false;
+#pragma unroll
+                    for (int r = 0; r < RY; ++r)
+                        if (k + 1 == S) rout[r] = make_uint2(0u, 0u);
                 } else {
+                    // rfa_advance() in full, two voxels per instruction (o - t and d - bv as exact-product FMAs)
+                    const u64 neg1 = pk(-1.0f, -1.0f), mg = pk(RFA_COMP_MAGIC, RFA_COMP_MAGIC), nmg = pk(-RFA_COMP_MAGIC, -RFA_COMP_MAGIC);
                     const unsigned plc = (unsigned)rfa_reflect(z0 - S + i - 1, P.nz) * plane4;   // level-0 centre plane
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
-                        const float4 c = q[k][CE][r];
-                        const float4 u = (r == 0) ? above : q[k][CE][r - 1];
-                        const float4 d = (r == RY - 1) ? below : q[k][CE][r + 1];
-                        float left = __shfl_up_sync(0xffffffffu, c.w, 1, TX);
-                        float right = __shfl_down_sync(0xffffffffu, c.x, 1, TX);
-                        if (xl_self) left = c.x;
-                        if (xr_self) right = c.w;
-                        const float4 zm = q[k][MI][r], zp = q[k][PH][r];
                         float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (hotq[k][CE]) {
                             if (k == 0) ri = unpack_h4(__ldg(rin2 + (plc + row_src[r])));
-                            else if (rvq[k][CE]) ri = unpack_h4(rsm[(((k - 1) * 2 + par_r) * RY + r) * NT + tid]);
+                            else if (rvq[k][CE]) ri = unpack_h4(rsm[(((k > 0 ? k - 1 : 0) * 2 + par_r) * RY + r) * NT + tid]);
                         }
-                        const uint32_t w = sw[r];
-                        const unsigned e0 = w & RFA_ST_INDEX, e1 = (w >> 8) & RFA_ST_INDEX, e2 = (w >> 16) & RFA_ST_INDEX,
-                                       e3 = (w >> 24) & RFA_ST_INDEX;
-                        float4 ro;
-                        rfa_advance(c.x, ri.x, tab[e0], rfa_bracket(c.x, left, c.y, u.x, d.x, zm.x, zp.x, tab[RFA_TABLE_N + e0], tab[2 * RFA_TABLE_N + e0], wx, wy, wz), o[r].x, ro.x);
-                        rfa_advance(c.y, ri.y, tab[e1], rfa_bracket(c.y, c.x, c.z, u.y, d.y, zm.y, zp.y, tab[RFA_TABLE_N + e1], tab[2 * RFA_TABLE_N + e1], wx, wy, wz), o[r].y, ro.y);
-                        rfa_advance(c.z, ri.z, tab[e2], rfa_bracket(c.z, c.y, c.w, u.z, d.z, zm.z, zp.z, tab[RFA_TABLE_N + e2], tab[2 * RFA_TABLE_N + e2], wx, wy, wz), o[r].z, ro.z);
-                        rfa_advance(c.w, ri.w, tab[e3], rfa_bracket(c.w, c.z, right, u.w, d.w, zm.w, zp.w, tab[RFA_TABLE_N + e3], tab[2 * RFA_TABLE_N + e3], wx, wy, wz), o[r].w, ro.w);
+                        u64 a01, a23, n01, n23, q01, q23, t01, t23, g01, g23;
+                        gather_row(r, a01, a23, n01, n23, q01, q23);
+                        bracket_row(r, n01, n23, q01, q23, t01, t23, g01, g23);
+                        const float4 c = q[k][CE][r];
+                        const bool h0 = fabsf(c.x) >= RFA_COMP_MIN, h1 = fabsf(c.y) >= RFA_COMP_MIN,
+                                   h2 = fabsf(c.z) >= RFA_COMP_MIN, h3 = fabsf(c.w) >= RFA_COMP_MIN;
+                        const u64 r01 = pk(h0 ? ri.x : 0.f, h1 ? ri.y : 0.f), r23 = pk(h2 ? ri.z : 0.f, h3 ? ri.w : 0.f);
+                        const u64 d01 = fma2(a01, g01, r01), d23 = fma2(a23, g23, r23);
+                        const u64 o01 = add2(t01, d01), o23 = add2(t23, d23);
+                        const u64 bv01 = fma2(t01, neg1, o01), bv23 = fma2(t23, neg1, o23);
+                        const u64 e01 = fma2(bv01, neg1, d01), e23 = fma2(bv23, neg1, d23);
+                        const u64 eq01 = add2(add2(e01, mg), nmg), eq23 = add2(add2(e23, mg), nmg);
+                        upk(o01, o[r].x, o[r].y);
+                        upk(o23, o[r].z, o[r].w);
                         mx = max_abs4(o[r], mx);
-                        const uint2 rp = pack_h4(ro.x, ro.y, ro.z, ro.w);
+                        float4 ro;
+                        upk(eq01, ro.x, ro.y);
+                        upk(eq23, ro.z, ro.w);
+                        const uint2 rp = pack_h4(h0 ? ro.x : 0.f, h1 ? ro.y : 0.f, h2 ? ro.z : 0.f, h3 ? ro.w : 0.f);
                         if (k + 1 < S) rsm[((k * 2 + par_w) * RY + r) * NT + tid] = rp;
                         else rout[r] = rp;
                     }
