@@ -39,7 +39,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "GVoxel-updates/s"
-STATE_BYTES_PER_VOXEL_PASS = 9.0     # 4 B theta read + 4 B theta write + 1 B packed state read
+STATE_BYTES_PER_VOXEL_PASS = 11.0    # 4 B theta read + 4 B theta write + 1 B state read + 2 B residual write
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
