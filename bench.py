@@ -40,6 +40,9 @@ if ROOT not in sys.path:
 
 METRIC = "GVoxel-updates/s"
 STATE_BYTES_PER_VOXEL_PASS = 11.0    # 4 B theta read + 4 B theta write + 1 B state read + 2 B residual write
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the one
+# `ncu --set full` capture committed under profiles/ (r1_blocked_s3_ncu_full.md); keyed by (config, fused steps)
+NCU_TRAFFIC_BYTES = {("C4", 3): 709.7e6}
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
@@ -269,7 +272,7 @@ def run_ours(args):
     achieved = bytes_per_launch / (launch_us * 1e-6) / 1e9
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": None, "peak_source": peak_src,
+        "traffic": NCU_TRAFFIC_BYTES.get((args.config, q1["fused_steps"])), "peak_source": peak_src,
         "kernel": f"rfa_blocked_kernel<S={q1['fused_steps']}>" if q1["kernel"] == binding.KERNEL_BLOCKED else "rfa_plain_kernel",
         "launches": launches, "avg_launch_us": launch_us, "algorithmic_bytes_per_launch": bytes_per_launch,
         "fused_steps_per_launch": q1["fused_steps"],

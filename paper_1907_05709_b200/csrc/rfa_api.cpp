@@ -54,7 +54,7 @@ struct rfa_sim {
     unsigned char *scratch = nullptr;    // nvox*4 bytes staging
     unsigned long long *counters = nullptr;
     int kernel = RFA_KERNEL_AUTO;
-    int fused = 2;
+    int fused = 3;
     RfaTbPlan plans[5]{};                // index = fused steps 1..4
     int resident[5]{};
     long long launches = 0;
@@ -452,7 +452,7 @@ extern "C" int rfa_configure(rfa_sim *s, int kernel, int fused_steps)
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
     if (kernel != RFA_KERNEL_AUTO && kernel != RFA_KERNEL_PLAIN && kernel != RFA_KERNEL_BLOCKED) return fail(RFA_E_INVALID, "bad kernel id %d", kernel);
     if (fused_steps < 0 || fused_steps > 4) return fail(RFA_E_INVALID, "fused_steps must be 0..4");
-    const int f = fused_steps == 0 ? 2 : fused_steps;
+    const int f = fused_steps == 0 ? 3 : fused_steps;
     if (kernel == RFA_KERNEL_BLOCKED && !s->plans[f].ok)
         return fail(RFA_E_INVALID, "the blocked kernel needs nx %% 4 == 0 and ny, nz >= fused steps (grid %dx%dx%d, fused %d)", s->g.nx, s->g.ny, s->g.nz, f);
     s->kernel = kernel;
