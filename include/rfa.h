@@ -132,6 +132,29 @@ int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launche
  * out = { ok, tiles_x, tiles_y, z_chunks, planes_per_chunk, work_items, ctas_launched, tile_bx, tile_by }. */
 int rfa_plan_query(const int dims[3], int batch, int fused_steps, int resident_ctas, int out[9]);
 
+/* ---- probe time series and frame hand-off ---------------------------------
+ * The paper reads temperatures at probe points 2.5 mm and 5 mm from the tip over 120 s (PAPER.md:147,
+ * Fig. 6 :250, Fig. 14 :282) and, per displayed frame, hands the finished buffer to the renderer while
+ * the next iteration runs into the other one (Alg. 2). */
+
+/* Set the probe points: n_probes flat voxel indices into the batched volume,
+ * index = scenario*nx*ny*nz + i + nx*(j + ny*k)  (host array, copied; n_probes = 0 clears them). */
+int rfa_set_probes(rfa_sim *s, int n_probes, const int64_t *index);
+
+/* Advance n steps and record the probe temperatures (deg C) after every `every` steps:
+ * out[m*n_probes + p] = T at probe p after (m+1)*every steps, m < n/every  (n must be a multiple of
+ * every; every >= 1).  `out` is host or device memory of (n/every)*n_probes floats.  The stepping uses
+ * the configured kernel (launches of up to fused_steps steps between records); the call returns after
+ * the records have arrived in `out`. */
+int rfa_step_record(rfa_sim *s, int n, int every, float *out);
+
+/* Frame hand-off (Alg. 2): device pointer of the finished image of one scenario as stored,
+ * theta = T - t_blood (fp32, nx*ny*nz, x fastest), and t_blood.  The image stays untouched by the NEXT
+ * launch of this simulation (it writes the other buffer) and is overwritten by the one after it: a
+ * consumer on another stream may read it while one more rfa_step launch (<= fused_steps time steps)
+ * runs.  The caller orders its read after the producing work (rfa_synchronize or a stream event). */
+int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_dev, float *t_blood_c);
+
 int rfa_synchronize(rfa_sim *s);
 void rfa_destroy(rfa_sim *s);
 const char *rfa_last_error(void);

@@ -158,6 +158,16 @@ class OracleSim:
                            int(n), _dp(self.T), _dp(self._buf), _up(self.necro))
         self.steps_done += int(n)
 
+    def step_record(self, n: int, every: int, index) -> np.ndarray:
+        """Probe time series (Fig. 6, Fig. 14): row m = T at the flat voxel indices after
+        (m+1)*every steps."""
+        idx = np.asarray(index, dtype=np.int64)
+        rows = []
+        for _ in range(int(n) // int(every)):
+            self.step(every)
+            rows.append(self.T.ravel()[idx].copy())
+        return np.array(rows, dtype=np.float64).reshape(len(rows), idx.size)
+
     # -- results ---------------------------------------------------------------------------
     def temperature(self) -> np.ndarray:
         return self.T.copy()

@@ -25,7 +25,8 @@ MAX_TISSUES = 32
 EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
-    "rfa_query", "rfa_plan_query", "rfa_synchronize", "rfa_destroy", "rfa_last_error",
+    "rfa_query", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
+    "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
 
 
@@ -82,6 +83,12 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_query.restype = ctypes.c_int
     lib.rfa_plan_query.argtypes = [i3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
     lib.rfa_plan_query.restype = ctypes.c_int
+    lib.rfa_set_probes.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int64)]
+    lib.rfa_set_probes.restype = ctypes.c_int
+    lib.rfa_step_record.argtypes = [vp, ctypes.c_int, ctypes.c_int, vp]
+    lib.rfa_step_record.restype = ctypes.c_int
+    lib.rfa_current_frame.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.POINTER(ctypes.c_float)]
+    lib.rfa_current_frame.restype = ctypes.c_int
     lib.rfa_synchronize.argtypes = [vp]
     lib.rfa_synchronize.restype = ctypes.c_int
     lib.rfa_destroy.argtypes = [vp]
@@ -218,6 +225,25 @@ class RfaSim:
         k, f, n = ctypes.c_int(), ctypes.c_int(), ctypes.c_int64()
         _check(self._lib.rfa_query(self._handle, ctypes.byref(k), ctypes.byref(f), ctypes.byref(n)))
         return {"kernel": int(k.value), "fused_steps": int(f.value), "kernel_launches": int(n.value)}
+
+    def set_probes(self, index):
+        idx = np.ascontiguousarray(index, dtype=np.int64).reshape(-1)
+        self.n_probes = int(idx.size)
+        _check(self._lib.rfa_set_probes(self._handle, self.n_probes,
+                                        idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)) if idx.size else None))
+
+    def step_record(self, n: int, every: int = 1, out=None):
+        rows = int(n) // max(int(every), 1)
+        if out is None:
+            out = np.empty((rows, getattr(self, "n_probes", 0)), dtype=np.float32)
+        _check(self._lib.rfa_step_record(self._handle, int(n), int(every), _ptr(out)))
+        return out
+
+    def current_frame(self, scenario: int = 0):
+        """(device address of theta = T - t_blood of the finished image, t_blood): Alg. 2 hand-off"""
+        p, tb = ctypes.c_void_p(), ctypes.c_float()
+        _check(self._lib.rfa_current_frame(self._handle, int(scenario), ctypes.byref(p), ctypes.byref(tb)))
+        return int(p.value), float(tb.value)
 
     def synchronize(self):
         _check(self._lib.rfa_synchronize(self._handle))

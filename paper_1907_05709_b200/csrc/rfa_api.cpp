@@ -58,6 +58,10 @@ struct rfa_sim {
     RfaTbPlan plans[5]{};                // index = fused steps 1..4
     int resident[5]{};
     long long launches = 0;
+    long long *probes = nullptr;         // device, n_probes flat voxel indices (library-owned)
+    int n_probes = 0;
+    float *record = nullptr;             // device staging of rfa_step_record (library-owned, grows on demand)
+    size_t record_cap = 0;               // floats
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -384,6 +388,8 @@ extern "C" void rfa_destroy(rfa_sim *s)
     if (!s) return;
     cudaStreamSynchronize(s->stream);
     if (s->own_ws) cudaFree(s->ws);
+    if (s->probes) cudaFree(s->probes);
+    if (s->record) cudaFree(s->record);
     delete s;
 }
 
@@ -470,10 +476,9 @@ extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *ker
     return RFA_OK;
 }
 
-extern "C" int rfa_step(rfa_sim *s, int n)
+// n time steps on the stream: launches of up to `fused` steps each, buffers swapped per launch (Alg. 2)
+static int advance(rfa_sim *s, int n)
 {
-    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
-    if (n < 0) return fail(RFA_E_INVALID, "n must be >= 0");
     const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
     while (n > 0) {
         cudaError_t e;
@@ -481,18 +486,95 @@ extern "C" int rfa_step(rfa_sim *s, int n)
         if (blocked) {
             did = std::min(n, s->fused);
             while (did > 1 && !s->plans[did].ok) --did;
-            if (s->plans[did].ok)
-                e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
-            else
-                e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
-        } else {
-            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
         }
+        if (blocked && s->plans[did].ok)
+            e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
+        else
+            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
         s->launches++;
         if (e != cudaSuccess) return cuda_fail(e, "step kernel");
         s->cur ^= 1;                                        // Alg. 2: swap the two buffers
         n -= did;
     }
+    return RFA_OK;
+}
+
+extern "C" int rfa_step(rfa_sim *s, int n)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (n < 0) return fail(RFA_E_INVALID, "n must be >= 0");
+    return advance(s, n);
+}
+
+extern "C" int rfa_set_probes(rfa_sim *s, int n_probes, const int64_t *index)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (n_probes < 0 || (n_probes > 0 && !index)) return fail(RFA_E_INVALID, "bad probe list");
+    const long long total = (long long)s->nvox * s->g.batch;
+    for (int p = 0; p < n_probes; ++p)
+        if (index[p] < 0 || index[p] >= total) return fail(RFA_E_INVALID, "probe %d: index %lld outside [0,%lld)", p, (long long)index[p], total);
+    cudaError_t e = cudaStreamSynchronize(s->stream);       // an earlier record may still read the old list
+    if (e != cudaSuccess) return cuda_fail(e, "set_probes");
+    if (s->probes) cudaFree(s->probes);
+    s->probes = nullptr;
+    s->n_probes = 0;
+    if (n_probes == 0) return RFA_OK;
+    e = cudaMalloc((void **)&s->probes, (size_t)n_probes * sizeof(long long));
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(RFA_E_NOMEM, "cudaMalloc of the probe list failed"); }
+    static_assert(sizeof(long long) == sizeof(int64_t), "probe indices are 64-bit");
+    e = cudaMemcpy(s->probes, index, (size_t)n_probes * sizeof(long long), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(e, "probe upload");
+    s->n_probes = n_probes;
+    return RFA_OK;
+}
+
+extern "C" int rfa_step_record(rfa_sim *s, int n, int every, float *out)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (n < 0 || every < 1 || (n % every) != 0) return fail(RFA_E_INVALID, "n must be a non-negative multiple of every >= 1");
+    if (s->n_probes == 0) return fail(RFA_E_INVALID, "no probes set (rfa_set_probes)");
+    if (!out) return fail(RFA_E_INVALID, "out is null");
+    const size_t rows = (size_t)(n / every), need = rows * (size_t)s->n_probes;
+    if (rows == 0) return RFA_OK;
+    const bool dev = is_device_ptr(out);
+    float *dst = out;
+    cudaError_t e;
+    if (!dev) {
+        if (s->record_cap < need) {
+            e = cudaStreamSynchronize(s->stream);
+            if (e != cudaSuccess) return cuda_fail(e, "step_record");
+            if (s->record) cudaFree(s->record);
+            s->record = nullptr;
+            s->record_cap = 0;
+            e = cudaMalloc((void **)&s->record, need * sizeof(float));
+            if (e != cudaSuccess) { cudaGetLastError(); return fail(RFA_E_NOMEM, "cudaMalloc of %zu record floats failed", need); }
+            s->record_cap = need;
+        }
+        dst = s->record;
+    }
+    for (size_t m = 0; m < rows; ++m) {
+        int rc = advance(s, every);
+        if (rc) return rc;
+        e = rfa_launch_probe(s->g, s->n_probes, s->probes, s->theta[s->cur], dst + m * s->n_probes, s->stream);
+        s->launches++;
+        if (e != cudaSuccess) return cuda_fail(e, "probe kernel");
+    }
+    if (!dev) {
+        e = cudaMemcpyAsync(out, dst, need * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "record download");
+    }
+    e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "step_record");
+    return RFA_OK;
+}
+
+extern "C" int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_dev, float *t_blood_c)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    if (!theta_dev) return fail(RFA_E_INVALID, "theta_dev is null");
+    *theta_dev = s->theta[s->cur] + (size_t)scenario * s->nvox;
+    if (t_blood_c) *t_blood_c = (float)s->t_blood;
     return RFA_OK;
 }
 

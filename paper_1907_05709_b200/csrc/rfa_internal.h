@@ -74,6 +74,8 @@ cudaError_t rfa_launch_get_temperature(const RfaGrid &g, int scenario, const flo
                                        cudaStream_t st);
 cudaError_t rfa_launch_get_necrosis(const RfaGrid &g, int scenario, const uint8_t *state, uint8_t *out_dev,
                                     cudaStream_t st);
+cudaError_t rfa_launch_probe(const RfaGrid &g, int n, const long long *index_dev, const float *theta /*all scenarios*/,
+                             float *out_dev, cudaStream_t st);
 cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *state, uint32_t label_held_mask,
                              unsigned long long *counters_dev /*2*/, cudaStream_t st);
 cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, const void *rin, void *rout,

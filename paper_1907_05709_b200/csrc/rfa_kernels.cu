@@ -112,6 +112,14 @@ __global__ void rfa_get_necrosis_kernel(size_t nvox, const uint8_t *__restrict__
     if (v < nvox) out[v] = state[v] >> 7;
 }
 
+// probe read-out (Fig. 6): T at n flat voxel indices of the batched volume
+__global__ void rfa_probe_kernel(int n, const long long *__restrict__ index, const float *__restrict__ theta,
+                                 float t_blood, float *__restrict__ out)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) out[p] = __fadd_rn(theta[index[p]], t_blood);
+}
+
 __global__ void rfa_count_kernel(size_t nvox, const uint8_t *__restrict__ state, uint32_t label_held_mask,
                                  unsigned long long *counters)
 {
@@ -639,6 +647,13 @@ cudaError_t rfa_launch_get_necrosis(const RfaGrid &g, int scenario, const uint8_
     return cudaGetLastError();
 }
 
+cudaError_t rfa_launch_probe(const RfaGrid &g, int n, const long long *index_dev, const float *theta, float *out_dev,
+                             cudaStream_t st)
+{
+    rfa_probe_kernel<<<blocks_for((size_t)n, 128), 128, 0, st>>>(n, index_dev, theta, g.t_blood, out_dev);
+    return cudaGetLastError();
+}
+
 cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *state, uint32_t label_held_mask,
                              unsigned long long *counters_dev, cudaStream_t st)
 {
@@ -721,8 +736,13 @@ static int resident_s()
     int dev = 0, sms = 0, occ = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::C::SMEM) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, K::C::NT, K::C::SMEM) != cudaSuccess) return 0;
+    // a shape that does not fit (shared memory, registers) yields 0 resident CTAs -> no plan for this S;
+    // the failed query must not stay behind as the runtime's sticky "last error"
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::C::SMEM) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, K::C::NT, K::C::SMEM) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
     return sms * occ;
 }
 

@@ -231,6 +231,44 @@ def c1_green(n: int = 64, h_mm: float = 1.0, dt: float = 0.1, steps: int = 1000,
 # ----------------------------------------------------------------------------------------------
 # C2 / C3: block phantoms in a 128 mm cube (BASELINE.json configs[1], [2])
 # ----------------------------------------------------------------------------------------------
+def fig6_probes(dims, spacing, centre_voxel, dists_mm=(2.5, 5.0)) -> np.ndarray:
+    """Flat voxel indices of the symmetric probe sets of PAPER.md:147 / Fig. 6: for each distance the six
+    points at +-d along x, y, z from the tip voxel (rounded to voxel centres).  Shape (len(dists), 6)."""
+    nx, ny, nz = dims
+    ci, cj, ck = centre_voxel
+    out = []
+    for d in dists_mm:
+        row = []
+        for a in range(3):
+            for sgn in (-1, 1):
+                o = [0, 0, 0]
+                o[a] = sgn * int(round(d / spacing[a]))
+                i, j, k = ci + o[0], cj + o[1], ck + o[2]
+                assert 0 <= i < nx and 0 <= j < ny and 0 <= k < nz, "probe outside the grid"
+                row.append(i + nx * (j + ny * k))
+        out.append(row)
+    return np.array(out, dtype=np.int64)
+
+
+def paper_probe_case(tip_c: float = 90.0, n: int = 64, steps: int = 1200) -> Workload:
+    """The paper's evaluation set-up: 0.5 mm grid, liver constants of :104 (with
+    Q_m), a 2.5 mm hemispherical tip (5 x 5 x 3 voxels) held at 90 or 60 C, dt = 0.1 s, 120 s."""
+    h = 0.5
+    labels = np.zeros((n, n, n), np.uint8)
+    c = n // 2
+    mask = np.zeros((n, n, n), np.uint8)
+    for dz in range(0, 3):
+        for dy in range(-2, 3):
+            for dx in range(-2, 3):
+                if (dx * dx + dy * dy + dz * dz) * h * h <= 1.25 * 1.25 + 1e-9:
+                    mask[c + dz, c + dy, c + dx] = 1
+    nd = Needle(mask=mask, mode=SRC_DIRICHLET, value=float(tip_c),
+                tip_mm=((c + 0.5) * h, (c + 0.5) * h, (c + 0.5) * h), axis=(0.0, 0.0, 1.0))
+    return Workload(name=f"paper_probe_{int(tip_c)}", dims=(n, n, n), spacing_mm=(h, h, h), labels=labels,
+                    table=paper_liver_table(), dt=0.1, steps=steps, needles=[nd],
+                    meta={"centre_voxel": (c, c, c)})
+
+
 def _block_phantom(c: int, n: int, h: float, n_tumours: int, n_vessels: int):
     rng = _rng(c)
     dims = (n, n, n)

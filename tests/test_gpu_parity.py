@@ -233,6 +233,63 @@ def test_monotone_and_bounded_on_gpu(rfa):
 
 
 # ----------------------------------------------------------------------------------------------
+# f2: probe time series (Fig. 6, Fig. 14) and the Alg. 2 frame hand-off
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("every,fused", [(1, 3), (6, 3), (4, 2)])
+def test_probe_series_matches_oracle(rfa, oracle, every, fused):
+    w = W.paper_probe_case(90.0, steps=240)
+    pr = W.fig6_probes(w.dims, w.spacing_mm, w.meta["centre_voxel"]).ravel()
+    osim = oracle.OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt)
+    osim.set_needle(w.needles[0].mask, w.needles[0].mode, w.needles[0].value)
+    exp = osim.step_record(w.steps, every, pr)
+    sim = rfa.from_workload(w)
+    sim.configure(rfa.KERNEL_BLOCKED, fused)
+    sim.set_probes(pr)
+    got = sim.step_record(w.steps, every)
+    assert got.shape == exp.shape == (w.steps // every, 12)
+    assert float(np.max(np.abs(got.astype(np.float64) - exp))) <= TOL
+    assert np.all(np.diff(got, axis=0) >= 0.0)            # monotone convergence, also in fp32
+    compare(sim.get_temperature(0), sim.get_necrosis(0), osim)   # the field itself after the recorded run
+    # device output buffer, probes cleared afterwards
+    import torch
+    dev_out = torch.empty((2, 12), dtype=torch.float32, device="cuda")
+    sim.step_record(2 * every, every, out=dev_out)
+    assert np.all(dev_out.cpu().numpy()[-1] >= got[-1])
+    sim.set_probes([])
+    with pytest.raises(rfa.RfaError):
+        sim.step_record(every, every)
+    sim.close()
+
+
+def test_frame_handoff_double_buffer(rfa):
+    """Alg. 2: the finished image stays intact while the next launch runs into the
+    other buffer, so a consumer on a second stream may read it concurrently."""
+    import torch
+    w = W.ragged_phantom(dims=(136, 70, 21), spacing=(0.7, 0.9, 1.3), steps=9, dt=0.05)
+    sim = rfa.from_workload(w)
+    sim.configure(rfa.KERNEL_BLOCKED, 3)
+    sim.step(9)
+    sim.synchronize()
+    want = sim.get_temperature(0)
+    ptr, t_blood = sim.current_frame(0)
+    nx, ny, nz = w.dims
+    side = torch.cuda.Stream()
+    host = torch.empty(nx * ny * nz, dtype=torch.float32, pin_memory=True)
+    sim.step(3)                                            # ONE more launch, asynchronous, writes the other buffer
+    from cuda.bindings import runtime as cudart           # raw device pointer -> pinned host, on the side stream
+    (rc,) = cudart.cudaMemcpyAsync(host.data_ptr(), ptr, host.numel() * 4,
+                                   cudart.cudaMemcpyKind.cudaMemcpyDeviceToHost, side.cuda_stream)
+    assert int(rc) == 0
+    side.synchronize()
+    sim.synchronize()
+    frame = host.numpy().reshape(nz, ny, nx)
+    assert np.array_equal((frame + np.float32(t_blood)).view(np.uint32), want.view(np.uint32))
+    ptr2, _ = sim.current_frame(0)
+    assert ptr2 != ptr                                     # the buffers were swapped by the launch
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------
 # Full-length configs against the stored oracle results (tests/golden/, written by make_golden.py)
 # ----------------------------------------------------------------------------------------------
 def _golden(name):

@@ -423,3 +423,36 @@ def test_golden_c2_is_reproducible_prefix(oracle):
     sim = oracle.run_workload(w, steps=int(g["checkpoints"][0]))
     got = sim.T.ravel()[g["sample_idx"]]
     assert np.array_equal(got, g["sample_T"][0])
+
+
+# ----------------------------------------------------------------------------------------------
+# Probe time series (SURVEY.md 8(f) f2; PAPER.md:147 Fig. 6 probe sets, :159 / Fig. 14 monotone convergence)
+# ----------------------------------------------------------------------------------------------
+def _probe_series(oracle, tip_c, steps=600, every=10):
+    w = W.paper_probe_case(tip_c, steps=steps)
+    pr = W.fig6_probes(w.dims, w.spacing_mm, w.meta["centre_voxel"])
+    sim = oracle.OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt)
+    nd = w.needles[0]
+    sim.set_needle(nd.mask, nd.mode, nd.value)
+    return sim.step_record(steps, every, pr.ravel()), pr
+
+
+def test_probe_series_monotone_symmetric_affine(oracle):
+    s90, pr = _probe_series(oracle, 90.0)
+    s60, _ = _probe_series(oracle, 60.0)
+    s75, _ = _probe_series(oracle, 75.0)
+    assert s90.shape == (60, 12)
+    # the paper's claim (Fig. 14): monotone convergence at the probes, from step 0 (R-18)
+    assert np.all(np.diff(s90, axis=0) >= -1e-12) and np.all(np.diff(s60, axis=0) >= -1e-12)
+    # Fig. 6: the +-x and +-y probes of one distance are equivalent by the symmetry of the hemispherical tip
+    # (x <-> y exactly; +x vs -x up to the wall reflection, the tip voxel is not the centre of an even box)
+    for base in (0, 6):
+        assert np.max(np.abs(s90[:, base + 0] - s90[:, base + 2])) < 1e-11
+        assert np.max(np.abs(s90[:, base + 1] - s90[:, base + 3])) < 1e-11
+        assert np.max(np.abs(s90[:, base + 0] - s90[:, base + 1])) < 1e-8
+    # the 2.5 mm set is hotter than the 5 mm set; the tip side (+z, inside/above the dome) is the hottest
+    assert np.all(s90[-1, :4] > s90[-1, 6:10]) and s90[-1, 5] > s90[-1, 0] > s90[-1, 4]
+    # the update is affine in the held tip value: T(75) = (T(90) + T(60)) / 2 at every probe and time
+    assert np.max(np.abs(s75 - 0.5 * (s90 + s60))) < 1e-11
+    # bounded by the tip temperature and by the far-field equilibrium T_a + Q_m / (w_b c_b) from below
+    assert s90.max() < 90.0 and s90.min() >= 37.0
