@@ -94,19 +94,83 @@ void rfa_oracle_step(int nx, int ny, int nz, double dx, double dy, double dz,
     }
 }
 
+/* One time step with CONSERVATIVE heterogeneous conduction (R-28):
+ * Eq. 9 writes div(K grad T) before Eq. 10/12 pull a constant K out of the divergence.
+ * Finite-volume form on the voxel grid: the heat flux through the face between voxel c and its face
+ * neighbour n is  Kf (T_n - T_c) / h  with the harmonic mean  Kf = 2 K_c K_n / (K_c + K_n)  of the two
+ * voxels' conductivities (two slabs of thickness h/2 in series), so
+ *   T_c' = T_c + dt/(rho c_p) * [ sum over the 6 faces Kf (T_n - T_c) / h_axis^2
+ *                                 + w_b c_b (T_a - T_c) + Q_m (+ Q) ]
+ * Outer grid faces carry no flux (the missing neighbour is the voxel itself, R-7).  Held voxels are
+ * copied and act on their neighbours through the face term with their own label's K.
+ * Arguments as rfa_oracle_step. */
+void rfa_oracle_step_cons(int nx, int ny, int nz, double dx, double dy, double dz,
+                          const uint8_t *lab, const uint8_t *held, const uint8_t *power,
+                          const double *K, const double *rho, const double *cp,
+                          const double *wb_cb, const double *q_m,
+                          double t_a, double q_power, double dt, double t_necro,
+                          const double *T, double *Tn, uint8_t *necro)
+{
+    int k;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (k = 0; k < nz; ++k) {
+        for (int j = 0; j < ny; ++j) {
+            for (int i = 0; i < nx; ++i) {
+                size_t v = (size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * (size_t)k);
+                double t = T[v];
+                double tn;
+                if (held[v]) {
+                    tn = t;
+                } else {
+                    int l = lab[v];
+                    double kc = K[l];
+                    double flux = 0.0;                     /* sum of Kf (T_n - T_c) / h^2 over the faces */
+                    for (int f = 0; f < 6; ++f) {
+                        int ii = i, jj = j, kk = k;
+                        double h;
+                        if (f == 0) { ii = i - 1; h = dx; }
+                        else if (f == 1) { ii = i + 1; h = dx; }
+                        else if (f == 2) { jj = j - 1; h = dy; }
+                        else if (f == 3) { jj = j + 1; h = dy; }
+                        else if (f == 4) { kk = k - 1; h = dz; }
+                        else { kk = k + 1; h = dz; }
+                        if (ii < 0 || ii >= nx || jj < 0 || jj >= ny || kk < 0 || kk >= nz) continue;   /* no flux */
+                        size_t n = (size_t)ii + (size_t)nx * ((size_t)jj + (size_t)ny * (size_t)kk);
+                        double kn = K[lab[n]];
+                        double kf = 2.0 * kc * kn / (kc + kn);
+                        flux += kf * (T[n] - t) / (h * h);
+                    }
+                    double rhs = flux + wb_cb[l] * (t_a - t) + q_m[l];
+                    if (power[v]) rhs += q_power;
+                    tn = t + dt / (rho[l] * cp[l]) * rhs;
+                }
+                Tn[v] = tn;
+                if (tn >= t_necro) necro[v] = 1;
+            }
+        }
+    }
+}
+
 /* nsteps iterations with the two buffers of Alg. 2.  On return the current
- * temperature image is in T (buf is scratch of the same size). */
+ * temperature image is in T (buf is scratch of the same size).  conservative != 0 selects
+ * rfa_oracle_step_cons (row f1), 0 the paper's Eq. 12 as printed. */
 void rfa_oracle_run(int nx, int ny, int nz, double dx, double dy, double dz,
                     const uint8_t *lab, const uint8_t *held, const uint8_t *power,
                     const double *K, const double *rho, const double *cp,
                     const double *wb_cb, const double *q_m,
                     double t_a, double q_power, double dt, double t_necro,
-                    int nsteps, double *T, double *buf, uint8_t *necro)
+                    int nsteps, double *T, double *buf, uint8_t *necro, int conservative)
 {
     double *a = T, *b = buf;
     for (int n = 0; n < nsteps; ++n) {
-        rfa_oracle_step(nx, ny, nz, dx, dy, dz, lab, held, power, K, rho, cp, wb_cb, q_m,
-                        t_a, q_power, dt, t_necro, a, b, necro);
+        if (conservative)
+            rfa_oracle_step_cons(nx, ny, nz, dx, dy, dz, lab, held, power, K, rho, cp, wb_cb, q_m,
+                                 t_a, q_power, dt, t_necro, a, b, necro);
+        else
+            rfa_oracle_step(nx, ny, nz, dx, dy, dz, lab, held, power, K, rho, cp, wb_cb, q_m,
+                            t_a, q_power, dt, t_necro, a, b, necro);
         double *t = a; a = b; b = t;
     }
     if (a != T) memcpy(T, a, sizeof(double) * (size_t)nx * (size_t)ny * (size_t)nz);

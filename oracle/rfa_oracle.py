@@ -57,7 +57,7 @@ def _load():
         common = [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [up, up, up] + [dp] * 5 + [ctypes.c_double] * 4
         lib.rfa_oracle_step.argtypes = common + [dp, dp, up]
         lib.rfa_oracle_step.restype = None
-        lib.rfa_oracle_run.argtypes = common + [ctypes.c_int, dp, dp, up]
+        lib.rfa_oracle_run.argtypes = common + [ctypes.c_int, dp, dp, up, ctypes.c_int]
         lib.rfa_oracle_run.restype = None
         lib.rfa_oracle_num_threads.restype = ctypes.c_int
         lib.rfa_oracle_set_num_threads.argtypes = [ctypes.c_int]
@@ -86,8 +86,9 @@ class OracleSim:
     k, rho, cp, wb_cb, q_m, t_init, flags; ``spacing_mm`` (dx, dy, dz) in millimetres (PAPER.md:115)."""
 
     def __init__(self, dims, spacing_mm, labels, table, t_blood: float, dt: float,
-                 t_necrosis: float = T_NECROSIS):
+                 t_necrosis: float = T_NECROSIS, conservative: bool = False):
         nx, ny, nz = (int(d) for d in dims)
+        self.conservative = bool(conservative)      # row f1: harmonic-mean face conductivities (R-28)
         self.dims = (nx, ny, nz)
         self.h_m = tuple(float(s) * 1.0e-3 for s in spacing_mm)     # mm -> m (R-2)
         self.lab = np.ascontiguousarray(labels, dtype=np.uint8).reshape(nz, ny, nx).copy()
@@ -155,7 +156,7 @@ class OracleSim:
                            _up(self.lab), _up(held), _up(self.power),
                            _dp(self.K), _dp(self.rho), _dp(self.cp), _dp(self.wb_cb), _dp(self.q_m),
                            self.t_a, self.q_power, self.dt, self.t_necro,
-                           int(n), _dp(self.T), _dp(self._buf), _up(self.necro))
+                           int(n), _dp(self.T), _dp(self._buf), _up(self.necro), int(self.conservative))
         self.steps_done += int(n)
 
     def step_record(self, n: int, every: int, index) -> np.ndarray:
@@ -188,12 +189,16 @@ class OracleSim:
         is a monotone (entrywise non-negative) map iff this is <= 1 (R-18)."""
         s = sum(1.0 / (h * h) for h in self.h_m)
         alpha = self.K / (self.rho * self.cp)
+        if self.conservative:
+            # worst face conductivity seen by a voxel of label l: 2 K_l K_max / (K_l + K_max)
+            kmax = float(self.K.max())
+            alpha = (2.0 * self.K * kmax / (self.K + kmax)) / (self.rho * self.cp)
         return float(np.max(self.dt * (2.0 * alpha * s + self.wb_cb / (self.rho * self.cp))))
 
 
-def run_workload(w, steps: int | None = None, scenario: int = 0) -> OracleSim:
+def run_workload(w, steps: int | None = None, scenario: int = 0, conservative: bool = False) -> OracleSim:
     """Run one scenario of a ``workloads.Workload`` for ``steps`` (default: the configured count)."""
-    sim = OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt)
+    sim = OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt, conservative=conservative)
     if w.t0 is not None:
         sim.set_temperature(w.t0)
     if w.needles:

@@ -456,3 +456,99 @@ def test_probe_series_monotone_symmetric_affine(oracle):
     assert np.max(np.abs(s75 - 0.5 * (s90 + s60))) < 1e-11
     # bounded by the tip temperature and by the far-field equilibrium T_a + Q_m / (w_b c_b) from below
     assert s90.max() < 90.0 and s90.min() >= 37.0
+
+
+# ----------------------------------------------------------------------------------------------
+# Row f1: conservative heterogeneous conduction div(K grad T) of Eq. 9, harmonic-mean
+# face conductivities (R-28).  Pins of rfa_oracle_step_cons.
+# ----------------------------------------------------------------------------------------------
+_MIX = [(0.21, 911.0, 2348.0, 0, 0, 37.0, 0), (0.512, 1060.0, 3600.0, 0, 0, 37.0, 0),
+        (0.53, 1050.0, 3700.0, 0, 0, 37.0, 0)]
+
+
+def test_cons_energy_is_conserved_with_mixed_tissues(oracle):
+    """The defining property of the conservative form (north_star: "energy conservation with zero-flux
+    boundaries and no sources"): sum_v rho c_p T_v is constant for ANY mix of tissues, which the
+    centre-K form of Eq. 12 does not give (test_weighted_energy_mixed_tissues)."""
+    dims = (10, 8, 6)
+    rng = np.random.default_rng(16)
+    table = W.make_table(_MIX)
+    lab = rng.integers(0, 3, size=(6, 8, 10)).astype(np.uint8)
+    T0 = 37.0 + 40.0 * rng.random((6, 8, 10))
+    sim = oracle.OracleSim(dims, (1.0, 0.7, 1.2), lab, table, 37.0, 0.05, conservative=True)
+    sim.set_temperature(T0)
+    rc = (table["rho"].astype(np.float64) * table["cp"])[lab]
+    sim.step(500)
+    e0, e1 = (rc * T0).sum(), (rc * sim.T).sum()
+    assert abs(e1 - e0) / e0 < 1e-13
+    assert np.ptp(sim.T) < np.ptp(T0)                       # and it diffuses
+    wgt = rc / table["k"].astype(np.float64)[lab]
+    assert abs((wgt * sim.T).sum() - (wgt * T0).sum()) / (wgt * T0).sum() > 1e-9   # the Eq. 12 invariant is not
+
+
+def test_cons_equals_eq12_when_homogeneous(oracle):
+    """One tissue (K constant): div(K grad T) = K lap T, so both forms must agree (Eq. 9 -> Eq. 10)."""
+    w = W.ragged_phantom(dims=(14, 11, 9), spacing=(0.7, 0.9, 1.3), steps=60, dt=0.05)
+    lab = np.where(w.labels == W.VESSEL, W.VESSEL, W.LIVER).astype(np.uint8)     # liver + held vessel, same K
+    a = oracle.OracleSim(w.dims, w.spacing_mm, lab, w.table, 37.0, w.dt)
+    b = oracle.OracleSim(w.dims, w.spacing_mm, lab, w.table, 37.0, w.dt, conservative=True)
+    for s in (a, b):
+        s.set_needle(w.needles[0].mask, W.SRC_DIRICHLET, 90.0)
+        s.step(60)
+    assert np.max(np.abs(a.T - b.T)) < 1e-11 and a.T.max() == 90.0
+
+
+def test_cons_two_layer_slab_is_series_resistors(oracle):
+    """1-D fat | liver slab between two held faces: the steady heat flux is (T_L - T_R) / sum(R) with
+    the thermal resistances h/K of the half-cells in series (textbook), and the temperature drops by
+    q R along the way.  The harmonic-mean face conductivity is exactly the two half-cells in series."""
+    n, m = 24, 10                                           # m fat voxels, then liver
+    table = W.make_table([(0.21, 911.0, 2348.0, 0, 0, 37.0, 0), (0.512, 1060.0, 3600.0, 0, 0, 37.0, 0),
+                          (0.21, 911.0, 2348.0, 0, 0, 80.0, W.TISSUE_HELD),
+                          (0.512, 1060.0, 3600.0, 0, 0, 37.0, W.TISSUE_HELD)])
+    lab = np.array([2] + [0] * (m - 1) + [1] * (n - m - 1) + [3], np.uint8).reshape(1, 1, n)
+    sim = oracle.OracleSim((n, 1, 1), (1.0, 1.0, 1.0), lab, table, 37.0, 1.0, conservative=True)
+    assert sim.stability_number() <= 1.0
+    sim.step(120000)
+    h = 1.0e-3
+    k_fat, k_liv = float(table["k"][0]), float(table["k"][1])   # the fp32 table values both sides are given
+    kv = np.array([k_fat] * m + [k_liv] * (n - m))
+    R = np.concatenate([[0.0], np.cumsum(0.5 * h / kv[:-1] + 0.5 * h / kv[1:])])   # centre-to-centre
+    q = (80.0 - 37.0) / R[-1]
+    assert np.max(np.abs(sim.T.ravel() - (80.0 - q * R))) < 1e-9
+    # the kink: slopes on the two sides are in the ratio K_liver / K_fat
+    T = sim.T.ravel()
+    assert abs((T[3] - T[4]) / (T[n - 5] - T[n - 4]) - k_liv / k_fat) < 1e-8
+
+
+def test_cons_operator_is_symmetric_stochastic_nonnegative(oracle):
+    """The one-step map A (columns = images of unit fields) of the conservative form: flux antisymmetry
+    makes diag(rho c_p)(A - I) symmetric, no-flux walls make every row sum to 1, and under the monotone
+    bound all entries are >= 0 (max principle)."""
+    dims = (5, 4, 3)
+    nx, ny, nz = dims
+    N = nx * ny * nz
+    rng = np.random.default_rng(3)
+    table = W.make_table(_MIX)
+    lab = rng.integers(0, 3, size=(nz, ny, nx)).astype(np.uint8)
+    A = np.zeros((N, N))
+    for j in range(N):
+        sim = oracle.OracleSim(dims, (0.7, 0.9, 1.3), lab, table, 0.0, 0.2, t_necrosis=1e9, conservative=True)
+        e = np.zeros(N)
+        e[j] = 1.0
+        sim.set_temperature(e.reshape(nz, ny, nx))
+        sim.step(1)
+        A[:, j] = sim.T.ravel()
+    rc = (table["rho"].astype(np.float64) * table["cp"])[lab].ravel()
+    M = rc[:, None] * (A - np.eye(N))
+    assert np.max(np.abs(M - M.T)) < 1e-9 * np.max(np.abs(M))
+    assert np.max(np.abs(A.sum(axis=1) - 1.0)) < 1e-14 and A.min() >= 0.0
+    # a fat|liver face couples the two voxels with dt * Kf / h^2 / (rho c_p), Kf = 2 K1 K2 / (K1 + K2)
+    found = False
+    for u in range(N - 1):
+        if (u % nx) < nx - 1 and {int(lab.ravel()[u]), int(lab.ravel()[u + 1])} == {0, 1}:
+            kf = 2 * 0.21 * 0.512 / (0.21 + 0.512)
+            assert abs(A[u, u + 1] * rc[u] - 0.2 * kf / (0.7e-3) ** 2) < 1e-6 * abs(A[u, u + 1] * rc[u])
+            found = True
+            break
+    assert found
