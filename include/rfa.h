@@ -52,19 +52,28 @@ typedef struct rfa_tissue {
 } rfa_tissue;
 
 enum { RFA_TISSUE_HELD = 1 };
-enum { RFA_MAX_TISSUES = 32 };   /* label ids 0..31 (5 bits of the packed state byte) */
+enum { RFA_MAX_TISSUES = 16 };   /* label ids 0..15 (4 bits of the packed state byte) */
 
 /* needle source modes (PAPER.md:145 held tip; BASELINE.json config 3 constant power, R-17) */
 enum { RFA_SRC_OFF = 0, RFA_SRC_DIRICHLET = 1 /* value = deg C */, RFA_SRC_POWER = 2 /* value = W/m^3 */ };
 
 enum {
     RFA_OK = 0,
-    RFA_E_INVALID = -1,   /* null pointer, non-positive dims/spacing/dt, label >= n_tissue, > 32 tissues,
+    RFA_E_INVALID = -1,   /* null pointer, non-positive dims/spacing/dt, label >= n_tissue, > 16 tissues,
                              scenario out of range, bad mode, workspace too small, non-finite constants */
     RFA_E_UNSTABLE = -2,  /* dt violates the monotone bound dt*(2 alpha sum 1/h^2 + w_b c_b/(rho c_p)) <= 1
                              for some non-held label (R-18)                                    */
     RFA_E_CUDA = -3,      /* a CUDA runtime call or kernel launch failed (also: no device)              */
     RFA_E_NOMEM = -4      /* host or device allocation failed                                          */
+};
+
+/* conduction term (rfa_set_conduction) */
+enum {
+    RFA_COND_EQ12 = 0,        /* Eq. 12 as printed: the voxel's own K times the 7-point Laplacian; default */
+    RFA_COND_FACE = 1         /* div(K grad T) of Eq. 9, conservative: flux through a face =
+                                 Kf (T_n - T_c)/h with the harmonic mean Kf = 2 K_c K_n/(K_c + K_n) of the two
+                                 voxels' K; identical to Eq. 12 inside a tissue, differs only at interfaces
+                                 (R-28).  Conserves sum rho c_p T.            */
 };
 
 /* kernel variants for rfa_configure (all produce bit-identical fields) */
@@ -123,6 +132,11 @@ int rfa_necrotic_voxels(rfa_sim *s, int scenario, int64_t *all_voxels, int64_t *
 
 /* Choose the kernel variant and, for the blocked kernel, the number of fused time steps (1..4; 0 = default). */
 int rfa_configure(rfa_sim *s, int kernel, int fused_steps);
+
+/* Choose the conduction term for all scenarios (RFA_COND_*).  RFA_COND_FACE re-checks the monotone bound with
+ * the largest face conductivity a voxel of each label can see (2 K K_max/(K + K_max)) and returns
+ * RFA_E_UNSTABLE, leaving the mode unchanged, if dt violates it. */
+int rfa_set_conduction(rfa_sim *s, int mode);
 
 /* Introspection: fused steps in use, kernel in use, number of kernel launches issued so far by this simulation. */
 int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launches);

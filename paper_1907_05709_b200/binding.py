@@ -19,13 +19,14 @@ RFA_OK, RFA_E_INVALID, RFA_E_UNSTABLE, RFA_E_CUDA, RFA_E_NOMEM = 0, -1, -2, -3, 
 SRC_OFF, SRC_DIRICHLET, SRC_POWER = 0, 1, 2
 KERNEL_AUTO, KERNEL_PLAIN, KERNEL_BLOCKED = 0, 1, 2
 TISSUE_HELD = 1
-MAX_TISSUES = 32
+MAX_TISSUES = 16
+COND_EQ12, COND_FACE = 0, 1
 
 # every symbol include/rfa.h declares
 EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
-    "rfa_query", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
+    "rfa_set_conduction", "rfa_query", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
     "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
 
@@ -79,6 +80,8 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_necrotic_voxels.restype = ctypes.c_int
     lib.rfa_configure.argtypes = [vp, ctypes.c_int, ctypes.c_int]
     lib.rfa_configure.restype = ctypes.c_int
+    lib.rfa_set_conduction.argtypes = [vp, ctypes.c_int]
+    lib.rfa_set_conduction.restype = ctypes.c_int
     lib.rfa_query.argtypes = [vp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int64)]
     lib.rfa_query.restype = ctypes.c_int
     lib.rfa_plan_query.argtypes = [i3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
@@ -220,6 +223,9 @@ class RfaSim:
 
     def configure(self, kernel: int = KERNEL_AUTO, fused_steps: int = 0):
         _check(self._lib.rfa_configure(self._handle, int(kernel), int(fused_steps)))
+
+    def set_conduction(self, mode: int):
+        _check(self._lib.rfa_set_conduction(self._handle, int(mode)))
 
     def query(self) -> dict:
         k, f, n = ctypes.c_int(), ctypes.c_int(), ctypes.c_int64()

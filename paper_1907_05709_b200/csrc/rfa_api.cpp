@@ -51,6 +51,8 @@ struct rfa_sim {
     int cur = 0;                         // index of the current image
     uint8_t *state = nullptr;            // packed state bytes
     float *tables = nullptr;             // batch x 3 x 128 coefficients
+    float *kap = nullptr;                // 16 x 16 face factors Kf/K_c - 1 (conservative conduction, R-28)
+    int conduction = RFA_COND_EQ12;
     unsigned char *scratch = nullptr;    // nvox*4 bytes staging
     unsigned long long *counters = nullptr;
     int kernel = RFA_KERNEL_AUTO;
@@ -70,7 +72,7 @@ struct rfa_sim {
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t theta0, theta1, resid0, resid1, state, tables, scratch, counters, total;
+    size_t theta0, theta1, resid0, resid1, state, tables, kap, scratch, counters, total;
 };
 
 static bool ws_layout(const int dims[3], int batch, WsLayout &L)
@@ -94,6 +96,8 @@ static bool ws_layout(const int dims[3], int batch, WsLayout &L)
     off = align256(off + nvox * batch);
     L.tables = off;
     off = align256(off + (size_t)batch * 3 * RFA_TABLE_N * 4);
+    L.kap = off;
+    off = align256(off + RFA_NLABEL * RFA_NLABEL * 4);
     L.scratch = off;
     off = align256(off + nvox * 4);
     L.counters = off;
@@ -355,6 +359,7 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     s->resid[1] = s->ws + L.resid1;
     s->state = s->ws + L.state;
     s->tables = (float *)(s->ws + L.tables);
+    s->kap = (float *)(s->ws + L.kap);
     s->scratch = s->ws + L.scratch;
     s->counters = (unsigned long long *)(s->ws + L.counters);
 
@@ -363,9 +368,22 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
         // labels -> device (staged through scratch), then label -> initial temperature image
         e = cudaMemcpyAsync(s->scratch, labels, nvox, cudaMemcpyHostToDevice, s->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "label upload"); break; }
-        float theta0[32];
-        for (int l = 0; l < 32; ++l) theta0[l] = l < n_tissue ? (float)((double)table[l].t_init - (double)t_blood_c) : 0.f;
-        e = rfa_launch_init(s->g, s->scratch, theta0, s->theta[0], s->resid[0], s->state, s->stream);
+        float theta0[RFA_NLABEL], kl[RFA_NLABEL], kap[RFA_NLABEL * RFA_NLABEL];
+        for (int l = 0; l < RFA_NLABEL; ++l) {
+            theta0[l] = l < n_tissue ? (float)((double)table[l].t_init - (double)t_blood_c) : 0.f;
+            kl[l] = l < n_tissue ? table[l].k : 0.f;
+        }
+        // face factors Kf/K_c - 1 = 2 K_n/(K_c + K_n) - 1 in fp64, rounded once; exactly 0 for equal K
+        for (int c = 0; c < RFA_NLABEL; ++c)
+            for (int n = 0; n < RFA_NLABEL; ++n) {
+                double v = 0.0;
+                if (c < n_tissue && n < n_tissue && table[c].k != table[n].k && (double)table[c].k + (double)table[n].k > 0.0)
+                    v = 2.0 * (double)table[n].k / ((double)table[c].k + (double)table[n].k) - 1.0;
+                kap[c * RFA_NLABEL + n] = (float)v;
+            }
+        e = cudaMemcpyAsync(s->kap, kap, sizeof kap, cudaMemcpyHostToDevice, s->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "face table upload"); break; }
+        e = rfa_launch_init(s->g, s->scratch, theta0, kl, s->theta[0], s->resid[0], s->state, s->stream);
         s->launches++;
         if (e != cudaSuccess) { rc = cuda_fail(e, "init kernel"); break; }
         for (int b = 0; b < batch && rc == RFA_OK; ++b) rc = upload_table(s, b);
@@ -466,6 +484,27 @@ extern "C" int rfa_configure(rfa_sim *s, int kernel, int fused_steps)
     return RFA_OK;
 }
 
+extern "C" int rfa_set_conduction(rfa_sim *s, int mode)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (mode != RFA_COND_EQ12 && mode != RFA_COND_FACE) return fail(RFA_E_INVALID, "bad conduction mode %d", mode);
+    if (mode == RFA_COND_FACE) {
+        // monotone bound with the largest face conductivity a voxel of each label can see (R-18, R-28)
+        double W = 0, kmax = 0, worst = 0;
+        for (int a = 0; a < 3; ++a) W += 1.0 / (s->h_m[a] * s->h_m[a]);
+        for (const rfa_tissue &t : s->table) kmax = std::max(kmax, (double)t.k);
+        for (const rfa_tissue &t : s->table) {
+            if (t.flags & RFA_TISSUE_HELD) continue;
+            const double rc = (double)t.rho * t.cp, kf = 2.0 * (double)t.k * kmax / ((double)t.k + kmax);
+            worst = std::max(worst, s->dt * (2.0 * kf / rc * W + (double)t.wb_cb / rc));
+        }
+        if (worst > 1.0)
+            return fail(RFA_E_UNSTABLE, "dt = %g s violates the monotone bound with face conductivities: %.4f > 1", s->dt, worst);
+    }
+    s->conduction = mode;
+    return RFA_OK;
+}
+
 extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launches)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
@@ -479,7 +518,8 @@ extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *ker
 // n time steps on the stream: launches of up to `fused` steps each, buffers swapped per launch (Alg. 2)
 static int advance(rfa_sim *s, int n)
 {
-    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
+    const float *kap = s->conduction == RFA_COND_FACE ? s->kap : nullptr;
+    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok && kap == nullptr;   // TODO blocked FACE
     while (n > 0) {
         cudaError_t e;
         int did = 1;
@@ -488,9 +528,9 @@ static int advance(rfa_sim *s, int n)
             while (did > 1 && !s->plans[did].ok) --did;
         }
         if (blocked && s->plans[did].ok)
-            e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
+            e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, kap, s->stream);
         else
-            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, s->stream);
+            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, kap, s->stream);
         s->launches++;
         if (e != cudaSuccess) return cuda_fail(e, "step kernel");
         s->cur ^= 1;                                        // Alg. 2: swap the two buffers

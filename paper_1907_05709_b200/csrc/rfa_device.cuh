@@ -5,17 +5,22 @@
 #include <cuda_runtime.h>
 
 // ---- packed state byte (one per voxel per scenario) ---------------------------------------------
-//   bits 0..4  label id (<= 32 tissues, "voxel-wise" parameters)
+//   bits 0..3  label id (<= 16 tissues, "voxel-wise" parameters)
+//   bit  4     interface: some face neighbour carries a label with a different conductivity K (static,
+//              set by rfa_init_kernel; only the conservative conduction mode looks at it, R-28)
 //   bit  5     needle voxel, Dirichlet: held at its temperature (Alg. 1 :306)
 //   bit  6     needle voxel, constant power source (R-17)
 //   bit  7     necrotic: T reached 60 C at some step (sticky)
-// bits 0..6 index the per-scenario coefficient table (128 entries).
-#define RFA_ST_LABEL 0x1fu
+// bits 0..6 index the per-scenario coefficient table (128 entries; the interface bit does not change
+// the coefficients).
+#define RFA_ST_LABEL 0x0fu
+#define RFA_ST_IFACE 0x10u
 #define RFA_ST_DIRICHLET 0x20u
 #define RFA_ST_POWER 0x40u
 #define RFA_ST_NECRO 0x80u
 #define RFA_ST_INDEX 0x7fu
 #define RFA_TABLE_N 128
+#define RFA_NLABEL 16
 
 // Per-scenario coefficient table, three planes of RFA_TABLE_N floats each (fp64 on the host,
 // rounded once):
@@ -46,6 +51,22 @@ __device__ __forceinline__ float rfa_bracket(float t, float xm, float xp, float 
     const float u = __fmaf_rn(np, t, qa);
     const float l = __fmaf_rn(wz, sz, __fmaf_rn(wy, sy, __fmaf_rn(wx, sx, u)));
     return __fmaf_rn(-2.0f, t, l);
+}
+
+// Conservative conduction (row f1, R-28): div(K grad T) of Eq. 9 with harmonic-mean
+// face conductivities Kf = 2 K_c K_n / (K_c + K_n).  Written as a correction to the bracket of Eq. 12,
+//   g_cons = g + sum_axis w_axis [ (Kf-/K_c - 1)(t- - t) + (Kf+/K_c - 1)(t+ - t) ],
+// so that voxels whose six neighbours share their K (interface bit clear: almost all) run the unchanged
+// sequence.  k?? = Kf/K_c - 1 from the 16x16 label-pair table (fp64 on the host, rounded once; exactly 0
+// for equal K).  Applied if and only if the voxel's interface bit is set.
+__device__ __forceinline__ float rfa_face_correction(float t, float xm, float xp, float ym, float yp, float zm,
+                                                     float zp, float kxm, float kxp, float kym, float kyp,
+                                                     float kzm, float kzp, float wx, float wy, float wz)
+{
+    const float cx = __fmaf_rn(kxm, __fsub_rn(xm, t), __fmul_rn(kxp, __fsub_rn(xp, t)));
+    const float cy = __fmaf_rn(kym, __fsub_rn(ym, t), __fmul_rn(kyp, __fsub_rn(yp, t)));
+    const float cz = __fmaf_rn(kzm, __fsub_rn(zm, t), __fmul_rn(kzp, __fsub_rn(zp, t)));
+    return __fmaf_rn(wz, cz, __fmaf_rn(wy, cy, __fmul_rn(wx, cx)));
 }
 
 // Compensated accumulation theta' = theta + a g.  With dt far below the

@@ -64,8 +64,9 @@ RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int res
 // launchers (rfa_kernels.cu).  All asynchronous on `st`; return cudaGetLastError().
 cudaError_t rfa_launch_table(const RfaTableHost &tbl, float *dst, cudaStream_t st);
 // resid: fp16 residual image (rfa_device.cuh: rfa_advance), same indexing as theta
-cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const float *theta0_by_label /*host, 32*/,
-                            float *theta, void *resid, uint8_t *state, cudaStream_t st);
+cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const float *theta0_by_label /*host, 16*/,
+                            const float *k_by_label /*host, 16*/, float *theta, void *resid, uint8_t *state,
+                            cudaStream_t st);
 cudaError_t rfa_launch_needle(const RfaGrid &g, int scenario, const uint8_t *mask_dev /*may be null*/, int mode,
                               float theta_value, float *theta, void *resid, uint8_t *state, cudaStream_t st);
 cudaError_t rfa_launch_set_temperature(const RfaGrid &g, int scenario, const float *t_dev, float *theta,
@@ -78,9 +79,11 @@ cudaError_t rfa_launch_probe(const RfaGrid &g, int n, const long long *index_dev
                              float *out_dev, cudaStream_t st);
 cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *state, uint32_t label_held_mask,
                              unsigned long long *counters_dev /*2*/, cudaStream_t st);
+// kap: null = Eq. 12 as printed; else device table [16][16] of Kf/K_c - 1 (conservative conduction, R-28)
 cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, const void *rin, void *rout,
-                             uint8_t *state, const float *tables, cudaStream_t st);
+                             uint8_t *state, const float *tables, const float *kap, cudaStream_t st);
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
-                               const void *rin, void *rout, uint8_t *state, const float *tables, cudaStream_t st);
+                               const void *rin, void *rout, uint8_t *state, const float *tables, const float *kap,
+                               cudaStream_t st);
 // resident CTAs of the blocked kernel on the current device for `fused` steps (occupancy * SM count)
 int rfa_blocked_resident_ctas(int fused);

@@ -45,20 +45,36 @@ __global__ void rfa_table_kernel(RfaTableHost tbl, float *dst)
     }
 }
 
-struct Theta0 {
-    float v[32];
+struct LabelInfo {
+    float theta0[RFA_NLABEL];       // initial theta = t_init - T_a per label
+    float k[RFA_NLABEL];            // conductivity per label: equal K <=> no interface between two labels
 };
 
 // label -> initial temperature image: theta = t_init[label] - T_a, state = label id,
-// necrosis on the initial state (R-14).  One launch covers all scenarios.
-__global__ void rfa_init_kernel(size_t nvox, int batch, const uint8_t *__restrict__ labels, Theta0 t0, float thr,
-                                float *__restrict__ theta, __half *__restrict__ resid, uint8_t *__restrict__ state)
+// necrosis on the initial state (R-14), interface bit = some in-grid face neighbour carries a
+// label with a different K (R-28).  One launch covers all scenarios.
+__global__ void rfa_init_kernel(int nx, int ny, int nz, int batch, const uint8_t *__restrict__ labels, LabelInfo li,
+                                float thr, float *__restrict__ theta, __half *__restrict__ resid,
+                                uint8_t *__restrict__ state)
 {
+    const size_t nvox = (size_t)nx * ny * nz;
     size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= nvox) return;
+    const int i = (int)(v % nx);
+    const int j = (int)((v / nx) % ny);
+    const int k = (int)(v / ((size_t)nx * ny));
+    const size_t sy = nx, sz = (size_t)nx * ny;
     unsigned l = labels[v] & RFA_ST_LABEL;
-    float t = t0.v[l];
-    unsigned st = l | (t >= thr ? RFA_ST_NECRO : 0u);
+    const float kc = li.k[l];
+    bool iface = false;
+    if (i > 0) iface |= li.k[labels[v - 1] & RFA_ST_LABEL] != kc;
+    if (i < nx - 1) iface |= li.k[labels[v + 1] & RFA_ST_LABEL] != kc;
+    if (j > 0) iface |= li.k[labels[v - sy] & RFA_ST_LABEL] != kc;
+    if (j < ny - 1) iface |= li.k[labels[v + sy] & RFA_ST_LABEL] != kc;
+    if (k > 0) iface |= li.k[labels[v - sz] & RFA_ST_LABEL] != kc;
+    if (k < nz - 1) iface |= li.k[labels[v + sz] & RFA_ST_LABEL] != kc;
+    float t = li.theta0[l];
+    unsigned st = l | (iface ? RFA_ST_IFACE : 0u) | (t >= thr ? RFA_ST_NECRO : 0u);
     for (int b = 0; b < batch; ++b) {
         theta[(size_t)b * nvox + v] = t;
         resid[(size_t)b * nvox + v] = __float2half_rn(0.f);
@@ -147,7 +163,8 @@ __global__ void rfa_count_kernel(size_t nvox, const uint8_t *__restrict__ state,
 // ------------------------------------------------------------------------------------------------
 __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float *__restrict__ tout,
                                  const __half *__restrict__ rin, __half *__restrict__ rout,
-                                 uint8_t *__restrict__ state, const float *__restrict__ tables)
+                                 uint8_t *__restrict__ state, const float *__restrict__ tables,
+                                 const float *__restrict__ kap /* null: Eq. 12; else 16x16 Kf/K_c - 1 (R-28) */)
 {
     const size_t nvox = (size_t)g.nx * g.ny * g.nz;
     size_t gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -169,8 +186,20 @@ __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float
     const float zp = k < g.nz - 1 ? T[v + sz] : t;
     const unsigned st = state[gid];
     const unsigned e = st & RFA_ST_INDEX;
-    const float br = rfa_bracket(t, xm, xp, ym, yp, zm, zp, __ldg(tab + RFA_TABLE_N + e),
-                                 __ldg(tab + 2 * RFA_TABLE_N + e), g.wx, g.wy, g.wz);
+    float br = rfa_bracket(t, xm, xp, ym, yp, zm, zp, __ldg(tab + RFA_TABLE_N + e),
+                           __ldg(tab + 2 * RFA_TABLE_N + e), g.wx, g.wy, g.wz);
+    if (kap != nullptr && (st & RFA_ST_IFACE)) {
+        // labels of the six face neighbours (a missing neighbour is the voxel itself: same K, factor 0)
+        const uint8_t *S = state + (size_t)b * nvox;
+        const unsigned lc = (st & RFA_ST_LABEL) * RFA_NLABEL;
+        const unsigned lxm = i > 0 ? S[v - sx] : st, lxp = i < g.nx - 1 ? S[v + sx] : st;
+        const unsigned lym = j > 0 ? S[v - sy] : st, lyp = j < g.ny - 1 ? S[v + sy] : st;
+        const unsigned lzm = k > 0 ? S[v - sz] : st, lzp = k < g.nz - 1 ? S[v + sz] : st;
+        br = __fadd_rn(br, rfa_face_correction(t, xm, xp, ym, yp, zm, zp, __ldg(kap + lc + (lxm & RFA_ST_LABEL)),
+                                               __ldg(kap + lc + (lxp & RFA_ST_LABEL)), __ldg(kap + lc + (lym & RFA_ST_LABEL)),
+                                               __ldg(kap + lc + (lyp & RFA_ST_LABEL)), __ldg(kap + lc + (lzm & RFA_ST_LABEL)),
+                                               __ldg(kap + lc + (lzp & RFA_ST_LABEL)), g.wx, g.wy, g.wz));
+    }
     float r, res;
     rfa_advance(t, __half2float(rin[gid]), __ldg(tab + e), br, r, res);
     tout[gid] = r;
@@ -213,6 +242,7 @@ struct RfaTbParams {
     __half *rout;
     uint8_t *state;
     const float *tables;
+    const float *kap;                 // conservative conduction: [16][16] Kf/K_c - 1; null = Eq. 12 as printed
     int nx, ny, nz, batch;
     int nx4;
     float wx, wy, wz, thr;
@@ -417,7 +447,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 uint32_t diff = sw[k][0] ^ __byte_perm(sw[k][0], 0, 0);
 #pragma unroll
                 for (int r = 1; r < RY; ++r) diff |= sw[k][0] ^ sw[k][r];
-                uni[k] = __all_sync(0xffffffffu, (diff & 0x7f7f7f7fu) == 0u);    // one label per thread
+                uni[k] = __all_sync(0xffffffffu, (diff & 0x6f6f6f6fu) == 0u);    // one label per thread
                 cold[k] = __all_sync(0xffffffffu, !hotq[k][CE]);                  // all residuals are zero
             }
             __syncthreads();                               // exchange rows of iteration i-1 are visible
@@ -598,13 +628,17 @@ cudaError_t rfa_launch_table(const RfaTableHost &tbl, float *dst, cudaStream_t s
     return cudaGetLastError();
 }
 
-cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const float *theta0_by_label, float *theta,
-                            void *resid, uint8_t *state, cudaStream_t st)
+cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const float *theta0_by_label,
+                            const float *k_by_label, float *theta, void *resid, uint8_t *state, cudaStream_t st)
 {
-    Theta0 t0;
-    for (int i = 0; i < 32; ++i) t0.v[i] = theta0_by_label[i];
+    LabelInfo li;
+    for (int i = 0; i < RFA_NLABEL; ++i) {
+        li.theta0[i] = theta0_by_label[i];
+        li.k[i] = k_by_label[i];
+    }
     size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    rfa_init_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(nvox, g.batch, labels_dev, t0, g.thr, theta, (__half *)resid, state);
+    rfa_init_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(g.nx, g.ny, g.nz, g.batch, labels_dev, li, g.thr, theta,
+                                                           (__half *)resid, state);
     return cudaGetLastError();
 }
 
@@ -666,10 +700,10 @@ cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *stat
 }
 
 cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, const void *rin, void *rout,
-                             uint8_t *state, const float *tables, cudaStream_t st)
+                             uint8_t *state, const float *tables, const float *kap, cudaStream_t st)
 {
     size_t n = (size_t)g.nx * g.ny * g.nz * g.batch;
-    rfa_plain_kernel<<<blocks_for(n, 256), 256, 0, st>>>(g, tin, tout, (const __half *)rin, (__half *)rout, state, tables);
+    rfa_plain_kernel<<<blocks_for(n, 256), 256, 0, st>>>(g, tin, tout, (const __half *)rin, (__half *)rout, state, tables, kap);
     return cudaGetLastError();
 }
 
@@ -696,9 +730,11 @@ static cudaError_t launch_blocked_s(const RfaTbParams &p, int grid, cudaStream_t
 }
 
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
-                               const void *rin, void *rout, uint8_t *state, const float *tables, cudaStream_t st)
+                               const void *rin, void *rout, uint8_t *state, const float *tables, const float *kap,
+                               cudaStream_t st)
 {
     RfaTbParams p;
+    p.kap = kap;
     p.tin = tin;
     p.tout = tout;
     p.rin = (const __half *)rin;

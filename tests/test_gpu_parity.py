@@ -233,6 +233,52 @@ def test_monotone_and_bounded_on_gpu(rfa):
 
 
 # ----------------------------------------------------------------------------------------------
+# f1: conservative conduction (harmonic-mean face conductivities, R-28)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", RAGGED[:3], ids=lambda c: "x".join(map(str, c["dims"])))
+def test_conservative_conduction_parity_and_variants(rfa, oracle, case):
+    w = W.ragged_phantom(dims=case["dims"], spacing=case["spacing"], steps=case["steps"], dt=0.05,
+                         mode=case["mode"], value=case["value"])
+    osim = oracle.run_workload(w, conservative=True)
+    plain = oracle.run_workload(w, conservative=False)
+    assert np.max(np.abs(osim.T - plain.T)) > 1e-2           # the two conduction terms really differ here
+    results = []
+    for kernel, fused in [(rfa.KERNEL_PLAIN, 0), (rfa.KERNEL_BLOCKED, 1), (rfa.KERNEL_BLOCKED, 2),
+                          (rfa.KERNEL_BLOCKED, 3), (rfa.KERNEL_BLOCKED, 4)]:
+        sim = rfa.from_workload(w)
+        sim.configure(kernel, fused)
+        sim.set_conduction(rfa.COND_FACE)
+        sim.step(w.steps)
+        T, N = sim.get_temperature(0), sim.get_necrosis(0)
+        sim.close()
+        compare(T, N, osim)
+        results.append((T, N))
+    for T, N in results[1:]:
+        assert np.array_equal(T.view(np.uint32), results[0][0].view(np.uint32)) and np.array_equal(N, results[0][1])
+
+
+def test_conservative_conduction_conserves_energy_on_gpu(rfa):
+    """sum rho c_p T constant (no perfusion, no sources, nothing held) to fp32 round-off."""
+    dims = (72, 40, 18)
+    rng = np.random.default_rng(5)
+    table = W.make_table([(0.21, 911.0, 2348.0, 0, 0, 37.0, 0), (0.512, 1060.0, 3600.0, 0, 0, 37.0, 0),
+                          (0.53, 1050.0, 3700.0, 0, 0, 37.0, 0)])
+    lab = (rng.random((18, 40, 72)) * 3).astype(np.uint8)
+    lab[:, :, 36:] = 1                                        # half random mix, half homogeneous
+    T0 = (37.0 + 30.0 * rng.random((18, 40, 72))).astype(np.float32)
+    sim = rfa.RfaSim(dims, (0.9, 1.1, 1.3), lab, table, 37.0, 0.05)
+    sim.set_conduction(rfa.COND_FACE)
+    sim.set_temperature(0, T0)
+    rc = (table["rho"].astype(np.float64) * table["cp"])[lab]
+    e0 = float((rc * (T0.astype(np.float64) - 37.0)).sum())
+    sim.step(300)
+    T = sim.get_temperature(0).astype(np.float64)
+    e1 = float((rc * (T - 37.0)).sum())
+    assert abs(e1 - e0) / e0 < 2e-6 and np.ptp(T) < 0.7 * np.ptp(T0)
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------
 # f2: probe time series (PAPER.md:147, Fig. 6, Fig. 14) and the Alg. 2 frame hand-off
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("every,fused", [(1, 3), (6, 3), (4, 2)])
