@@ -140,13 +140,14 @@ def _needle_slab(w, nzc):
     return z0, nzc
 
 
-def oracle_time(w, steps, warmup, nzc):
+def oracle_time(w, steps, warmup, nzc, conservative=False):
     """Times `steps` oracle time steps on a z-slab of w (full slab = whole volume when nzc >= nz)."""
     from oracle import rfa_oracle
     rfa_oracle.build()
     nx, ny, nz = w.dims
     z0, nzc = _needle_slab(w, nzc)
-    sim = rfa_oracle.OracleSim((nx, ny, nzc), w.spacing_mm, w.labels[z0:z0 + nzc], w.table, w.t_blood, w.dt)
+    sim = rfa_oracle.OracleSim((nx, ny, nzc), w.spacing_mm, w.labels[z0:z0 + nzc], w.table, w.t_blood, w.dt,
+                               conservative=conservative)
     if w.needles:
         nd = w.needles[0]
         sim.set_needle(nd.mask[z0:z0 + nzc], nd.mode, nd.value)
@@ -158,11 +159,11 @@ def oracle_time(w, steps, warmup, nzc):
     return secs, nx * ny * nzc, rfa_oracle.num_threads(), (z0, nzc)
 
 
-def cpu_baseline(w, budget_s=15.0):
+def cpu_baseline(w, budget_s=15.0, conservative=False):
     """The oracle, as it stands, on a bounded sample: whole volume, as many time steps as fit ~budget_s."""
-    secs1, nv, thr, _ = oracle_time(w, 1, 0, w.dims[2])
+    secs1, nv, thr, _ = oracle_time(w, 1, 0, w.dims[2], conservative)
     n = int(max(1, min(50, budget_s / max(secs1, 1e-3))))
-    secs, nv, thr, _ = oracle_time(w, n, 0, w.dims[2])
+    secs, nv, thr, _ = oracle_time(w, n, 0, w.dims[2], conservative)
     gv = nv * n / secs / 1e9
     return {"value": gv, "unit": METRIC, "cores": thr, "kind": "oracle",
             "sample": f"{n} time steps of the full {w.dims[0]}x{w.dims[1]}x{w.dims[2]} {w.name} volume, fp64, "
@@ -178,11 +179,12 @@ def run_reference(args):
     w = W.BENCH_CONFIGS[args.config]()
     nx, ny, nz = w.dims
     # calibrate on a thin slab, then size the slab so K + W steps end within ~budget seconds
-    secs, nv, thr, _ = oracle_time(w, 2, 1, min(nz, 8))
+    cons = args.conduction == "face"
+    secs, nv, thr, _ = oracle_time(w, 2, 1, min(nz, 8), cons)
     rate = nv * 2 / secs
     budget = 100.0
     nzc = int(max(1, min(nz, budget * rate / ((args.steps + args.warmup) * nx * ny))))
-    secs, nv, thr, (z0, nzc) = oracle_time(w, args.steps, args.warmup, nzc)
+    secs, nv, thr, (z0, nzc) = oracle_time(w, args.steps, args.warmup, nzc, cons)
     gv = nv * args.steps / secs / 1e9
     sample = (f"{args.steps} time steps on the z-slab [{z0},{z0 + nzc}) of {w.name} ({nx}x{ny}x{nzc} voxels around "
               f"the needle), fp64 oracle, OpenMP over z")
@@ -239,6 +241,8 @@ def run_ours(args):
     with torch.cuda.stream(stream):
         sim = binding.from_workload(w, device=dev, stream=stream)
         sim.configure(args.kernel, args.fused)
+        if args.conduction == "face":
+            sim.set_conduction(binding.COND_FACE)
         sim.step(Wu)
         sim.synchronize()
         q0 = sim.query()
@@ -295,6 +299,8 @@ def run_ours(args):
             s2 = binding.RfaSim(w.dims, w.spacing_mm, lab_h, w.table, w.t_blood, w.dt, batch=w.batch,
                                 device=dev, stream=stream)
             s2.configure(args.kernel, args.fused)
+            if args.conduction == "face":
+                s2.set_conduction(binding.COND_FACE)
             for b, nd in enumerate(w.needles):
                 s2.set_needle(b, masks[b], nd.mode, nd.value, nd.tip_mm, nd.axis)
             s2.step(K)
@@ -316,7 +322,7 @@ def run_ours(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        cpu = cpu_baseline(w)
+        cpu = cpu_baseline(w, conservative=(args.conduction == "face"))
 
     if rank == 0:
         line = {
@@ -328,7 +334,7 @@ def run_ours(args):
                        "l2": "inputs larger than L2 (2 x %d MiB fields + %d MiB state vs 126 MB L2)" % (
                            nvox_all * 4 >> 20, nvox_all >> 20) if nvox_all * 9 > 126e6 * 2 else
                              "working set fits L2 (reported, not held to the HBM bar)",
-                       "kernel": roofline["kernel"]},
+                       "kernel": roofline["kernel"], "conduction": args.conduction},
             "sim_steps_per_s": K / (ms * 1e-3) * (1 if world == 1 else world),
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
             "clocks": clk.summary(),
@@ -346,9 +352,11 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=12000)
     ap.add_argument("--warmup", type=int, default=120)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5", "C4F"])
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 plain, 2 blocked (rfa_configure)")
     ap.add_argument("--fused", type=int, default=0, help="fused time steps per launch, 0 = library default")
+    ap.add_argument("--conduction", default="eq12", choices=["eq12", "face"],
+                    help="eq12: Eq. 12 as printed (default, the headline); face: conservative div(K grad T), row f1")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args(argv)

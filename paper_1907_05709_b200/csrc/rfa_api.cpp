@@ -519,7 +519,7 @@ extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *ker
 static int advance(rfa_sim *s, int n)
 {
     const float *kap = s->conduction == RFA_COND_FACE ? s->kap : nullptr;
-    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok && kap == nullptr;   // TODO blocked FACE
+    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
     while (n > 0) {
         cudaError_t e;
         int did = 1;

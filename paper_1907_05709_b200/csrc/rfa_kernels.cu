@@ -251,21 +251,24 @@ struct RfaTbParams {
 
 constexpr int rfa_pow2_at_least(int n) { return n <= 1 ? 1 : 2 * rfa_pow2_at_least((n + 1) / 2); }
 
-template <int S, int TX, int TY, int RY>
+template <int S, int TX, int TY, int RY, bool CONS = false>
 struct TbCfg {
     static constexpr int NT = TX * TY;
     static constexpr int BX = 4 * TX;
     static constexpr int BY = RY * TY;
     static constexpr int PD = 1;                                  // prefetch distance (planes in flight)
     static constexpr int DT = 2;                                  // temperature ring depth (PD + 1)
-    static constexpr int DS = rfa_pow2_at_least(PD + S + 1);      // state ring depth (level k reads plane i-k-1)
+    // state ring depth: level k reads plane i-k-1; the conservative mode also reads the planes i-k and i-k-2 and
+    // the rows of the neighbouring threads (one extra slot keeps a thread one barrier ahead off them)
+    static constexpr int DS = rfa_pow2_at_least(CONS ? PD + S + 3 : PD + S + 1);
     static constexpr int NR = S > 1 ? S - 1 : 1;                  // inter-level residual buffers
     static constexpr size_t RING_T = (size_t)DT * RY * NT * 16;
     static constexpr size_t EXCH = (size_t)S * 2 * 2 * NT * 16;
     static constexpr size_t RING_S = (size_t)DS * RY * NT * 4;
     static constexpr size_t RSM = (size_t)NR * 2 * RY * NT * 8;
     static constexpr size_t TAB = 3 * RFA_TABLE_N * 4;
-    static constexpr size_t SMEM = RING_T + EXCH + RING_S + RSM + TAB;
+    static constexpr size_t KAP = CONS ? RFA_NLABEL * RFA_NLABEL * 4 : 0;
+    static constexpr size_t SMEM = RING_T + EXCH + RING_S + RSM + TAB + KAP;
 };
 
 typedef unsigned long long u64;
@@ -305,15 +308,44 @@ __device__ __forceinline__ float4 unpack_h4(const uint2 v)
     return make_float4(lo.x, lo.y, hi.x, hi.y);
 }
 
+// Conservative conduction, one row of four voxels (rfa_device.cuh: rfa_face_correction; R-28): g of
+// every voxel whose interface bit is set gets the face correction added.  w = the row's state word, w?? = the
+// state words of its six neighbour rows aligned byte for byte, kap = [16][16] face factors in shared memory.
+// Inlined on purpose: a __noinline__ version (smaller SASS) was slower on the B200 (298 vs 380 GVox/s on C4):
+// the call ABI forces spills in a kernel that already sits at the 128-register cap.
+__device__ __forceinline__ float4 rfa_face_row(float4 g, const float4 c, const float4 u, const float4 d, const float4 zm,
+                                            const float4 zp, const float left, const float right, const uint32_t w,
+                                            const uint32_t wxm, const uint32_t wxp, const uint32_t wym,
+                                            const uint32_t wyp, const uint32_t wzm, const uint32_t wzp,
+                                            const float *kap, const float wx, const float wy, const float wz)
+{
+    float gg[4] = {g.x, g.y, g.z, g.w};
+    const float tc[4] = {c.x, c.y, c.z, c.w}, txm[4] = {left, c.x, c.y, c.z}, txp[4] = {c.y, c.z, c.w, right},
+                tym[4] = {u.x, u.y, u.z, u.w}, typ[4] = {d.x, d.y, d.z, d.w}, tzm[4] = {zm.x, zm.y, zm.z, zm.w},
+                tzp[4] = {zp.x, zp.y, zp.z, zp.w};
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        if ((w >> (8 * v)) & RFA_ST_IFACE) {
+            const float *kc = kap + ((w >> (8 * v)) & RFA_ST_LABEL) * RFA_NLABEL;
+            gg[v] = __fadd_rn(gg[v], rfa_face_correction(tc[v], txm[v], txp[v], tym[v], typ[v], tzm[v], tzp[v],
+                                                         kc[(wxm >> (8 * v)) & RFA_ST_LABEL], kc[(wxp >> (8 * v)) & RFA_ST_LABEL],
+                                                         kc[(wym >> (8 * v)) & RFA_ST_LABEL], kc[(wyp >> (8 * v)) & RFA_ST_LABEL],
+                                                         kc[(wzm >> (8 * v)) & RFA_ST_LABEL], kc[(wzp >> (8 * v)) & RFA_ST_LABEL],
+                                                         wx, wy, wz));
+        }
+    }
+    return make_float4(gg[0], gg[1], gg[2], gg[3]);
+}
+
 template <int I>
 struct IC {
     static constexpr int value = I;
 };
 
-template <int S, int TX, int TY, int RY, int MINB>
+template <int S, int TX, int TY, int RY, int MINB, bool CONS>
 __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbParams P)
 {
-    using C = TbCfg<S, TX, TY, RY>;
+    using C = TbCfg<S, TX, TY, RY, CONS>;
     constexpr int NT = C::NT, BX = C::BX, BY = C::BY, PD = C::PD, DT = C::DT, DS = C::DS;
     static_assert(RY == 4 || RY == 2, "state words of a thread are read as one vector");
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -322,6 +354,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
     uint32_t *ringS = reinterpret_cast<uint32_t *>(smem_raw + C::RING_T + C::EXCH);                // [DS][NT][RY]
     uint2 *rsm = reinterpret_cast<uint2 *>(smem_raw + C::RING_T + C::EXCH + C::RING_S);            // [NR][2 parity][RY][NT]
     float *tab = reinterpret_cast<float *>(smem_raw + C::RING_T + C::EXCH + C::RING_S + C::RSM);   // [3][128]
+    float *kap = tab + 3 * RFA_TABLE_N;                                                            // [16][16] (CONS)
 
     const int tid = threadIdx.x;
     const int tx = tid % TX, ty = tid / TX;
@@ -329,6 +362,8 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
     const int dn_tid = (ty < TY - 1 ? ty + 1 : ty) * TX + tx;
 
     for (int e = tid; e < S * 2 * 2 * NT; e += NT) exch[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if constexpr (CONS)
+        for (int e = tid; e < RFA_NLABEL * RFA_NLABEL; e += NT) kap[e] = P.kap[e];
 
     const unsigned plane4 = (unsigned)(P.ny * P.nx4);       // float4 (= state words = residual quads) per plane
     const float wx = P.wx, wy = P.wy, wz = P.wz;
@@ -433,7 +468,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
             // state words of the S centre planes and the two warp votes per level that pick the code path:
             // thread-private data, so all of it is issued before the barrier and overlaps the wait
             uint32_t sw[S][RY];
-            bool uni[S], cold[S];
+            bool uni[S], cold[S], ifc[S];
 #pragma unroll
             for (int k = 0; k < S; ++k) {
                 const int sS = (i - (k + 1)) & (DS - 1);
@@ -447,7 +482,15 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 uint32_t diff = sw[k][0] ^ __byte_perm(sw[k][0], 0, 0);
 #pragma unroll
                 for (int r = 1; r < RY; ++r) diff |= sw[k][0] ^ sw[k][r];
-                uni[k] = __all_sync(0xffffffffu, (diff & 0x6f6f6f6fu) == 0u);    // one label per thread
+                bool one = (diff & 0x6f6f6f6fu) == 0u;                           // one label per thread
+                if constexpr (CONS) {                                            // ... and no interface voxel
+                    uint32_t any = sw[k][0];
+#pragma unroll
+                    for (int r = 1; r < RY; ++r) any |= sw[k][r];
+                    ifc[k] = __any_sync(0xffffffffu, (any & 0x10101010u) != 0u); // some voxel of the warp needs face terms
+                    one = one && !ifc[k];
+                }
+                uni[k] = __all_sync(0xffffffffu, one);
                 cold[k] = __all_sync(0xffffffffu, !hotq[k][CE]);                  // all residuals are zero
             }
             __syncthreads();                               // exchange rows of iteration i-1 are visible
@@ -467,7 +510,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
 
                 // g = rfa_bracket() of the four voxels of row r, two voxels per instruction
                 auto bracket_row = [&](const int r, const u64 n01, const u64 n23, const u64 q01, const u64 q23,
-                                       u64 &t01, u64 &t23, u64 &g01, u64 &g23) {
+                                       u64 &t01, u64 &t23, u64 &g01, u64 &g23, const bool faces) {
                     const float4 c = q[k][CE][r];
                     const float4 u = (r == 0) ? above : q[k][CE][r > 0 ? r - 1 : 0];
                     const float4 d = (r == RY - 1) ? below : q[k][CE][r < RY - 1 ? r + 1 : r];
@@ -486,6 +529,28 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                     const u64 l23 = fma2(wz2, sz23, fma2(wy2, sy23, fma2(wx2, sx23, fma2(n23, t23, q23))));
                     g01 = fma2(m2, t01, l01);
                     g23 = fma2(m2, t23, l23);
+                    if constexpr (CONS) {
+                        if (faces) {
+                            // conservative conduction (R-28): labels of the six face neighbours of the row's four
+                            // voxels as byte-aligned words; rfa_face_correction() where the interface bit is set
+                            const uint32_t w = sw[k][r];
+                            const uint32_t wl = __shfl_up_sync(0xffffffffu, w, 1, TX), wr = __shfl_down_sync(0xffffffffu, w, 1, TX);
+                            const uint32_t wxm = (w << 8) | (xl_self ? (w & 0xffu) : (wl >> 24));
+                            const uint32_t wxp = (w >> 8) | (xr_self ? (w & 0xff000000u) : (wr << 24));
+                            const int sC = (i - (k + 1)) & (DS - 1), sM = (i - (k + 2)) & (DS - 1), sP = (i - k) & (DS - 1);
+                            const uint32_t wym = (r == 0) ? ringS[(sC * NT + up_tid) * RY + RY - 1] : sw[k][r > 0 ? r - 1 : 0];
+                            const uint32_t wyp = (r == RY - 1) ? ringS[(sC * NT + dn_tid) * RY] : sw[k][r < RY - 1 ? r + 1 : r];
+                            const uint32_t wzm = ringS[(sM * NT + tid) * RY + r], wzp = ringS[(sP * NT + tid) * RY + r];
+                            if (w & 0x10101010u) {
+                                float4 gg;
+                                upk(g01, gg.x, gg.y);
+                                upk(g23, gg.z, gg.w);
+                                gg = rfa_face_row(gg, c, u, d, zm, zp, left, right, w, wxm, wxp, wym, wyp, wzm, wzp, kap, wx, wy, wz);
+                                g01 = pk(gg.x, gg.y);
+                                g23 = pk(gg.z, gg.w);
+                            }
+                        }
+                    }
                 };
                 // per-voxel coefficients of row r (tissue interfaces, needle voxels)
                 auto gather_row = [&](const int r, u64 &a01, u64 &a23, u64 &n01, u64 &n23, u64 &q01, u64 &q23) {
@@ -509,7 +574,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
 #pragma unroll
                         for (int r = 0; r < RY; ++r) {
                             u64 t01, t23, g01, g23;
-                            bracket_row(r, n2, n2, q2, q2, t01, t23, g01, g23);
+                            bracket_row(r, n2, n2, q2, q2, t01, t23, g01, g23, false);
                             upk(add2(t01, fma2(a2, g01, zero2)), o[r].x, o[r].y);
                             upk(add2(t23, fma2(a2, g23, zero2)), o[r].z, o[r].w);
                             mx = max_abs4(o[r], mx);
@@ -519,7 +584,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                         for (int r = 0; r < RY; ++r) {
                             u64 a01, a23, n01, n23, q01, q23, t01, t23, g01, g23;
                             gather_row(r, a01, a23, n01, n23, q01, q23);
-                            bracket_row(r, n01, n23, q01, q23, t01, t23, g01, g23);
+                            bracket_row(r, n01, n23, q01, q23, t01, t23, g01, g23, CONS && ifc[k]);
                             upk(add2(t01, fma2(a01, g01, zero2)), o[r].x, o[r].y);
                             upk(add2(t23, fma2(a23, g23, zero2)), o[r].z, o[r].w);
                             mx = max_abs4(o[r], mx);
@@ -542,7 +607,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                         }
                         u64 a01, a23, n01, n23, q01, q23, t01, t23, g01, g23;
                         gather_row(r, a01, a23, n01, n23, q01, q23);
-                        bracket_row(r, n01, n23, q01, q23, t01, t23, g01, g23);
+                        bracket_row(r, n01, n23, q01, q23, t01, t23, g01, g23, CONS && ifc[k]);
                         const float4 c = q[k][CE][r];
                         const bool h0 = fabsf(c.x) >= RFA_COMP_MIN, h1 = fabsf(c.y) >= RFA_COMP_MIN,
                                    h2 = fabsf(c.z) >= RFA_COMP_MIN, h3 = fabsf(c.w) >= RFA_COMP_MIN;
@@ -707,17 +772,17 @@ cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, co
     return cudaGetLastError();
 }
 
-template <int S>
+template <int S, bool CONS>
 struct TbKernel {
     static constexpr RfaTbShape sh = RFA_TB_SHAPE[S];
-    using C = TbCfg<S, sh.tx, sh.ty, sh.ry>;
-    static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb>; }
+    using C = TbCfg<S, sh.tx, sh.ty, sh.ry, CONS>;
+    static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb, CONS>; }
 };
 
-template <int S>
-static cudaError_t launch_blocked_s(const RfaTbParams &p, int grid, cudaStream_t st)
+template <int S, bool CONS>
+static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_t st)
 {
-    using K = TbKernel<S>;
+    using K = TbKernel<S, CONS>;
     auto kern = K::get();
     static bool attr_set = false;
     if (!attr_set) {
@@ -727,6 +792,12 @@ static cudaError_t launch_blocked_s(const RfaTbParams &p, int grid, cudaStream_t
     }
     kern<<<grid, K::C::NT, K::C::SMEM, st>>>(p);
     return cudaGetLastError();
+}
+
+template <int S>
+static cudaError_t launch_blocked_s(const RfaTbParams &p, int grid, cudaStream_t st)
+{
+    return p.kap != nullptr ? launch_blocked_sc<S, true>(p, grid, st) : launch_blocked_sc<S, false>(p, grid, st);
 }
 
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
@@ -767,7 +838,7 @@ cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const fl
 template <int S>
 static int resident_s()
 {
-    using K = TbKernel<S>;
+    using K = TbKernel<S, true>;            // the conservative variant needs the larger state ring: plan for it
     auto kern = K::get();
     int dev = 0, sms = 0, occ = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;

@@ -453,4 +453,19 @@ def ragged_phantom(dims=(45, 38, 29), spacing=(0.7, 0.9, 1.3), seed: int = 7, dt
     return Workload(f"ragged{dims}", tuple(dims), tuple(spacing), labels, table, dt, steps, needles)
 
 
-BENCH_CONFIGS = {"C1": c1_cube, "C2": c2_phantom, "C3": c3_phantom, "C4": c4_body, "C5": c5_sweep}
+def c4_face_case(steps: int = 400) -> Workload:
+    """C4 body model with a smooth non-uniform initial temperature (37 + 8 cos cos cos, deg C), so that heat
+    crosses every tissue interface from the first step: the full-size case of the conservative conduction
+    term (row f1).  Needle as in C4."""
+    w = c4_body(steps=steps)
+    nx, ny, nz = w.dims
+    cx = np.cos(2.0 * np.pi * (np.arange(nx) + 0.5) / 64.0)
+    cy = np.cos(2.0 * np.pi * (np.arange(ny) + 0.5) / 48.0)
+    cz = np.cos(2.0 * np.pi * (np.arange(nz) + 0.5) / 32.0)
+    w.t0 = 37.0 + 8.0 * cz[:, None, None] * cy[None, :, None] * cx[None, None, :]
+    w.name = "C4F"
+    return w
+
+
+BENCH_CONFIGS = {"C1": c1_cube, "C2": c2_phantom, "C3": c3_phantom, "C4": c4_body, "C5": c5_sweep,
+                 "C4F": c4_face_case}

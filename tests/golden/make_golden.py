@@ -13,7 +13,9 @@ and for the final state: a 32^3 crop around the needle centroid (crop_lo, crop_T
 necrosis mask, necrotic voxel counts (all / without held-label and needle voxels), the voxels whose
 temperature lies within 2e-3 C of 60 C (band_idx, band_T: the exempt band of BASELINE.json's
 north_star is 1e-3), the field sum and maximum, a fingerprint of the inputs, and the oracle's speed.
-For the batched config C5 the same is stored per scenario (fewer samples each).
+For the batched config C5 the same is stored per scenario (fewer samples each).  "C4F" = the C4 body model with a
+smooth non-uniform initial field and the conservative conduction term (row f1), 400 steps, with extra
+samples on tissue interfaces.
 """
 from __future__ import annotations
 
@@ -57,12 +59,26 @@ def sample_indices(w, scenario: int, n: int, seed: int) -> np.ndarray:
     return np.unique(np.concatenate([near, far]).astype(np.int64))
 
 
-def run_scenario(w, scenario: int, n_samples: int, crop: int, checkpoints):
+def interface_indices(w, n: int, seed: int) -> np.ndarray:
+    """Flat indices of voxels whose +x neighbour carries a different label (tissue interfaces), a seeded subset."""
+    lab = w.labels
+    z, y, x = np.nonzero(lab[:, :, :-1] != lab[:, :, 1:])
+    rng = np.random.Generator(np.random.PCG64(seed))
+    pick = rng.choice(len(z), size=min(n, len(z)), replace=False)
     nx, ny, nz = w.dims
-    sim = rfa_oracle.OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt)
+    return (x[pick] + nx * (y[pick] + ny * z[pick])).astype(np.int64)
+
+
+def run_scenario(w, scenario: int, n_samples: int, crop: int, checkpoints, conservative: bool = False):
+    nx, ny, nz = w.dims
+    sim = rfa_oracle.OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt, conservative=conservative)
+    if w.t0 is not None:
+        sim.set_temperature(w.t0)
     nd = w.needles[scenario]
     sim.set_needle(nd.mask, nd.mode, nd.value)
     idx = sample_indices(w, scenario, n_samples, 190705709 + 17 * scenario + len(w.name))
+    if conservative:
+        idx = np.unique(np.concatenate([idx, interface_indices(w, n_samples, 190705709 + 99)]))
     out_T = []
     prev = None
     done = 0
@@ -71,7 +87,7 @@ def run_scenario(w, scenario: int, n_samples: int, crop: int, checkpoints):
         sim.step(cp - done)
         done = cp
         cur = sim.T.ravel()[idx].copy()
-        if prev is not None:      # constant heating from T_a: non-decreasing
+        if prev is not None and w.t0 is None:      # constant heating from T_a: non-decreasing
             assert np.all(cur >= prev - 1e-12), "oracle field not monotone between checkpoints"
         prev = cur
         out_T.append(cur)
@@ -113,12 +129,14 @@ def main():
     if args.threads:
         rfa_oracle.set_num_threads(args.threads)
     for name in args.configs:
+        # "C4F" = the C4 body model with a non-uniform initial field, conservative conduction term (row f1)
+        cons = name.endswith("F")
         w = W.BENCH_CONFIGS[name]()
         cps = [w.steps // 4, w.steps // 2, w.steps]
         print(f"{name}: dims {w.dims} steps {w.steps} batch {w.batch}", flush=True)
         out = {"dims": np.array(w.dims), "checkpoints": np.array(cps), "batch": np.int64(w.batch)}
         if w.batch == 1:
-            out.update(run_scenario(w, 0, 4096, 32, cps))
+            out.update(run_scenario(w, 0, 4096, 32, cps, conservative=cons))
         else:
             for b in range(w.batch):
                 r = run_scenario(w, b, 512, 16, [w.steps])
