@@ -346,6 +346,46 @@ def run_ours(args):
     return 0
 
 
+def run_warp(args):
+    """Row f3 (Eq. 14 warp) on the C4 volume: K warps of the heated image through a device-resident displacement
+    field; algorithmic bytes per voxel = 12 (displacement) + 4 (image, read once through L2) + 4 (output)."""
+    import torch
+    from paper_1907_05709_b200 import binding, workloads as W
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    w = W.BENCH_CONFIGS[args.config]()
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        sim = binding.from_workload(w, device=dev, stream=stream)
+        sim.step(300)
+        d = torch.from_numpy(W.breathing_field(w.dims)).to(dev)
+        out = torch.empty((w.dims[2], w.dims[1], w.dims[0]), dtype=torch.float32, device=dev)
+        for _ in range(max(args.warmup, 3)):
+            sim.warp_temperature(0, d, 0.85, out=out)
+        K = min(args.steps, 200)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with ClockSampler(dev.index or 0) as clk:
+            e0.record(stream)
+            for _ in range(K):
+                sim.warp_temperature(0, d, 0.85, out=out)
+            e1.record(stream)
+            e1.synchronize()
+        ms = float(e0.elapsed_time(e1))
+        sim.close()
+    peak, peak_src = measured_peak()
+    gv = w.n_voxels * K / (ms * 1e-3) / 1e9
+    ach = 20.0 * w.n_voxels * K / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "GVoxel/s (Eq. 14 warp)", "value": gv, "unit": "GVoxel/s", "n_gpus": 1, "steps": K,
+                      "warmup": max(args.warmup, 3), "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": w.name + " warp", "dims": list(w.dims), "field": "breathing_field, scale 0.85"},
+                      "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                                   "traffic": None, "peak_source": peak_src, "kernel": "rfa_warp_kernel",
+                                   "algorithmic_bytes_per_launch": 20.0 * w.n_voxels},
+                      "gpu_launches": K, "clocks": clk.summary()}), flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -357,6 +397,8 @@ def main(argv=None):
     ap.add_argument("--fused", type=int, default=0, help="fused time steps per launch, 0 = library default")
     ap.add_argument("--conduction", default="eq12", choices=["eq12", "face"],
                     help="eq12: Eq. 12 as printed (default, the headline); face: conservative div(K grad T), row f1")
+    ap.add_argument("--op", default="step", choices=["step", "warp"],
+                    help="step: the time-stepping hot path (the headline); warp: the Eq. 14 motion warp (row f3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args(argv)
@@ -364,6 +406,8 @@ def main(argv=None):
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.op == "warp":
+        return run_warp(args)
     return run_ours(args)
 
 

@@ -169,6 +169,18 @@ int rfa_step_record(rfa_sim *s, int n, int every, float *out);
  * runs.  The caller orders its read after the producing work (rfa_synchronize or a stream event). */
 int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_dev, float *t_blood_c);
 
+/* ---- breathing-motion warp (Eq. 14) -----------------------
+ * T(x_t) = T_ref(x_t + u^-1(x_t, t)): the temperature shown at position x_t of the moving anatomy is the
+ * reference-frame temperature looked up through the (inverse) motion field of the current breathing phase.
+ *   disp   host or device, 3*nx*ny*nz floats: the displacement field in MILLIMETRES as three volumes
+ *          (u_x, then u_y, then u_z; each x fastest like every volume)
+ *   scale  factor applied to the field (the breathing amplitude of the phase, "interpolated" :133)
+ *   out    host or device, nx*ny*nz floats, deg C:
+ *          out[v] = trilinear interpolation of the current temperature image of `scenario` at the position
+ *          (voxel centre of v) + scale*disp[v], sample positions clamped to the volume of voxel centres.
+ * Reads the simulation state, does not change it.  Synchronous (waits for the stream). */
+int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp, float scale, float *out);
+
 int rfa_synchronize(rfa_sim *s);
 void rfa_destroy(rfa_sim *s);
 const char *rfa_last_error(void);

@@ -27,6 +27,7 @@ EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
     "rfa_set_conduction", "rfa_query", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
+    "rfa_warp_temperature",
     "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
 
@@ -92,6 +93,8 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_step_record.restype = ctypes.c_int
     lib.rfa_current_frame.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.POINTER(ctypes.c_float)]
     lib.rfa_current_frame.restype = ctypes.c_int
+    lib.rfa_warp_temperature.argtypes = [vp, ctypes.c_int, vp, ctypes.c_float, vp]
+    lib.rfa_warp_temperature.restype = ctypes.c_int
     lib.rfa_synchronize.argtypes = [vp]
     lib.rfa_synchronize.restype = ctypes.c_int
     lib.rfa_destroy.argtypes = [vp]
@@ -250,6 +253,15 @@ class RfaSim:
         p, tb = ctypes.c_void_p(), ctypes.c_float()
         _check(self._lib.rfa_current_frame(self._handle, int(scenario), ctypes.byref(p), ctypes.byref(tb)))
         return int(p.value), float(tb.value)
+
+    def warp_temperature(self, scenario: int, disp, scale: float = 1.0, out=None):
+        """Eq. 14: the temperature image seen through a displacement field (3, nz, ny, nx) in mm"""
+        nx, ny, nz = self.dims
+        d = disp if not isinstance(disp, np.ndarray) else np.ascontiguousarray(disp, dtype=np.float32)
+        if out is None:
+            out = np.empty((nz, ny, nx), dtype=np.float32)
+        _check(self._lib.rfa_warp_temperature(self._handle, int(scenario), _ptr(d), float(scale), _ptr(out)))
+        return out
 
     def synchronize(self):
         _check(self._lib.rfa_synchronize(self._handle))

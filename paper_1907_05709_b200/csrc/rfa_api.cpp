@@ -618,6 +618,36 @@ extern "C" int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_d
     return RFA_OK;
 }
 
+extern "C" int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp, float scale, float *out)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    if (!disp || !out) return fail(RFA_E_INVALID, "null argument");
+    if (!std::isfinite(scale)) return fail(RFA_E_INVALID, "scale must be finite");
+    const size_t nvox = s->nvox;
+    const float *ddev = disp;
+    float *tmp = nullptr;
+    cudaError_t e;
+    if (!is_device_ptr(disp)) {
+        e = cudaMalloc((void **)&tmp, 3 * nvox * sizeof(float));
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(RFA_E_NOMEM, "cudaMalloc of the displacement staging failed"); }
+        e = cudaMemcpyAsync(tmp, disp, 3 * nvox * sizeof(float), cudaMemcpyHostToDevice, s->stream);
+        if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(e, "displacement upload"); }
+        ddev = tmp;
+    }
+    const bool dev = is_device_ptr(out);
+    float *dst = dev ? out : (float *)s->scratch;
+    const float inv_h[3] = {(float)(1.0e-3 / s->h_m[0]), (float)(1.0e-3 / s->h_m[1]), (float)(1.0e-3 / s->h_m[2])};
+    e = rfa_launch_warp(s->g, scenario, s->theta[s->cur], ddev, scale, inv_h, dst, s->stream);
+    s->launches++;
+    if (e == cudaSuccess && !dev) e = cudaMemcpyAsync(out, dst, nvox * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
+    cudaError_t e2 = cudaStreamSynchronize(s->stream);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) return cuda_fail(e, "warp kernel");
+    if (e2 != cudaSuccess) return cuda_fail(e2, "warp_temperature");
+    return RFA_OK;
+}
+
 extern "C" int rfa_synchronize(rfa_sim *s)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");

@@ -75,6 +75,8 @@ cudaError_t rfa_launch_get_temperature(const RfaGrid &g, int scenario, const flo
                                        cudaStream_t st);
 cudaError_t rfa_launch_get_necrosis(const RfaGrid &g, int scenario, const uint8_t *state, uint8_t *out_dev,
                                     cudaStream_t st);
+cudaError_t rfa_launch_warp(const RfaGrid &g, int scenario, const float *theta /*all scenarios*/, const float *disp_dev,
+                            float scale, const float inv_h_mm[3], float *out_dev, cudaStream_t st);
 cudaError_t rfa_launch_probe(const RfaGrid &g, int n, const long long *index_dev, const float *theta /*all scenarios*/,
                              float *out_dev, cudaStream_t st);
 cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *state, uint32_t label_held_mask,

@@ -128,6 +128,66 @@ __global__ void rfa_get_necrosis_kernel(size_t nvox, const uint8_t *__restrict__
     if (v < nvox) out[v] = state[v] >> 7;
 }
 
+// breathing-motion warp, Eq. 14: out[v] = T(x_v + scale * u[v]), trilinear, clamped (row f3).
+// The displacement is split into integer and fractional voxels BEFORE the voxel index is added, so the
+// interpolation weights keep the full fp32 resolution of the (small) displacement, not of the coordinate.
+__device__ __forceinline__ float rfa_warp_voxel(int i, int j, int k, int nx, int ny, int nz, const float *__restrict__ theta,
+                                                float dx, float dy, float dz, float t_blood)
+{
+    const float d[3] = {dx, dy, dz};
+    const int base[3] = {i, j, k}, n[3] = {nx, ny, nz};
+    int i0[3], i1[3];
+    float a[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float f = floorf(d[c]);
+        float frac = d[c] - f;
+        // clamp the shift first: |f| beyond the grid size saturates (and keeps the int conversion defined)
+        int p = base[c] + (int)fminf(fmaxf(f, -(float)n[c]), (float)n[c]);
+        if (p < 0) { p = 0; frac = 0.f; }
+        if (p >= n[c] - 1) { p = n[c] - 1; frac = 0.f; }
+        i0[c] = p;
+        i1[c] = min(p + 1, n[c] - 1);
+        a[c] = frac;
+    }
+    const size_t sy = nx, sz = (size_t)nx * ny;
+    const float *z0 = theta + (size_t)i0[2] * sz, *z1 = theta + (size_t)i1[2] * sz;
+    const size_t r0 = (size_t)i0[1] * sy, r1 = (size_t)i1[1] * sy;
+    const float c000 = __ldg(z0 + r0 + i0[0]), c100 = __ldg(z0 + r0 + i1[0]), c010 = __ldg(z0 + r1 + i0[0]),
+                c110 = __ldg(z0 + r1 + i1[0]), c001 = __ldg(z1 + r0 + i0[0]), c101 = __ldg(z1 + r0 + i1[0]),
+                c011 = __ldg(z1 + r1 + i0[0]), c111 = __ldg(z1 + r1 + i1[0]);
+    const float x00 = fmaf(a[0], c100 - c000, c000), x10 = fmaf(a[0], c110 - c010, c010);
+    const float x01 = fmaf(a[0], c101 - c001, c001), x11 = fmaf(a[0], c111 - c011, c011);
+    const float y0 = fmaf(a[1], x10 - x00, x00), y1 = fmaf(a[1], x11 - x01, x01);
+    return fmaf(a[2], y1 - y0, y0) + t_blood;
+}
+
+// grid = (x blocks, ny, nz): no integer division per voxel; VEC = 4 voxels per thread along x with 16-byte loads of
+// the three displacement components and a 16-byte store (nx % 4 == 0), VEC = 1 for any nx
+template <int VEC>
+__global__ void rfa_warp_kernel(int nx, int ny, int nz, const float *__restrict__ theta, const float *__restrict__ disp,
+                                float scale, float ihx, float ihy, float ihz, float t_blood, float *__restrict__ out)
+{
+    const int i = (blockIdx.x * blockDim.x + threadIdx.x) * VEC;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    if (i >= nx || j >= ny) return;
+    const size_t nvox = (size_t)nx * ny * nz;
+    const size_t v = (size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * k);
+    if constexpr (VEC == 4) {
+        const float4 ux = *reinterpret_cast<const float4 *>(disp + v), uy = *reinterpret_cast<const float4 *>(disp + nvox + v),
+                     uz = *reinterpret_cast<const float4 *>(disp + 2 * nvox + v);
+        float4 o;
+        o.x = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, scale * ux.x * ihx, scale * uy.x * ihy, scale * uz.x * ihz, t_blood);
+        o.y = rfa_warp_voxel(i + 1, j, k, nx, ny, nz, theta, scale * ux.y * ihx, scale * uy.y * ihy, scale * uz.y * ihz, t_blood);
+        o.z = rfa_warp_voxel(i + 2, j, k, nx, ny, nz, theta, scale * ux.z * ihx, scale * uy.z * ihy, scale * uz.z * ihz, t_blood);
+        o.w = rfa_warp_voxel(i + 3, j, k, nx, ny, nz, theta, scale * ux.w * ihx, scale * uy.w * ihy, scale * uz.w * ihz, t_blood);
+        *reinterpret_cast<float4 *>(out + v) = o;
+    } else {
+        out[v] = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, scale * disp[v] * ihx, scale * disp[nvox + v] * ihy,
+                                scale * disp[2 * nvox + v] * ihz, t_blood);
+    }
+}
+
 // probe read-out (Fig. 6): T at n flat voxel indices of the batched volume
 __global__ void rfa_probe_kernel(int n, const long long *__restrict__ index, const float *__restrict__ theta,
                                  float t_blood, float *__restrict__ out)
@@ -743,6 +803,22 @@ cudaError_t rfa_launch_get_necrosis(const RfaGrid &g, int scenario, const uint8_
 {
     size_t nvox = (size_t)g.nx * g.ny * g.nz;
     rfa_get_necrosis_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(nvox, state + (size_t)scenario * nvox, out_dev);
+    return cudaGetLastError();
+}
+
+cudaError_t rfa_launch_warp(const RfaGrid &g, int scenario, const float *theta, const float *disp_dev, float scale,
+                            const float inv_h_mm[3], float *out_dev, cudaStream_t st)
+{
+    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    const float *th = theta + (size_t)scenario * nvox;
+    const bool vec = (g.nx % 4) == 0 && (((uintptr_t)disp_dev | (uintptr_t)out_dev) & 15) == 0;
+    if (g.ny > 65535 * 4 || g.nz > 65535) return cudaErrorInvalidValue;
+    const dim3 block(64, 4, 1);
+    const dim3 grid((unsigned)((g.nx + (vec ? 256 : 64) - 1) / (vec ? 256 : 64)), (unsigned)((g.ny + 3) / 4), (unsigned)g.nz);
+    if (vec)
+        rfa_warp_kernel<4><<<grid, block, 0, st>>>(g.nx, g.ny, g.nz, th, disp_dev, scale, inv_h_mm[0], inv_h_mm[1], inv_h_mm[2], g.t_blood, out_dev);
+    else
+        rfa_warp_kernel<1><<<grid, block, 0, st>>>(g.nx, g.ny, g.nz, th, disp_dev, scale, inv_h_mm[0], inv_h_mm[1], inv_h_mm[2], g.t_blood, out_dev);
     return cudaGetLastError();
 }
 

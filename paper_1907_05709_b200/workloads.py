@@ -453,6 +453,22 @@ def ragged_phantom(dims=(45, 38, 29), spacing=(0.7, 0.9, 1.3), seed: int = 7, dt
     return Workload(f"ragged{dims}", tuple(dims), tuple(spacing), labels, table, dt, steps, needles)
 
 
+def breathing_field(dims, amp_mm=(2.0, 4.0, 12.0)) -> np.ndarray:
+    """Synthetic smooth displacement field (3, nz, ny, nx) in mm standing in for the paper's 4D-CT motion fields
+    (not available): mostly cranio-caudal (z), strongest mid-volume, vanishing at the z ends, varying
+    smoothly across x and y.  Scaled by the breathing amplitude of the phase by the caller."""
+    nx, ny, nz = dims
+    sz = np.sin(np.pi * (np.arange(nz, dtype=np.float32) + 0.5) / nz)[:, None, None]
+    cy = (0.6 + 0.4 * np.cos(2.0 * np.pi * (np.arange(ny, dtype=np.float32) + 0.5) / ny))[None, :, None]
+    sx = (0.8 + 0.2 * np.sin(2.0 * np.pi * (np.arange(nx, dtype=np.float32) + 0.5) / nx))[None, None, :]
+    base = (sz * cy * sx).astype(np.float32)
+    out = np.empty((3, nz, ny, nx), np.float32)
+    out[0] = amp_mm[0] * base * np.cos(np.pi * (np.arange(ny, dtype=np.float32) + 0.5) / ny)[None, :, None]
+    out[1] = -amp_mm[1] * base
+    out[2] = amp_mm[2] * base
+    return out
+
+
 def c4_face_case(steps: int = 400) -> Workload:
     """C4 body model with a smooth non-uniform initial temperature (37 + 8 cos cos cos, deg C), so that heat
     crosses every tissue interface from the first step: the full-size case of the conservative conduction

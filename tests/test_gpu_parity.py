@@ -336,6 +336,55 @@ def test_frame_handoff_double_buffer(rfa):
 
 
 # ----------------------------------------------------------------------------------------------
+# f3: breathing-motion warp, Eq. 14
+# ----------------------------------------------------------------------------------------------
+def test_warp_matches_oracle_elementwise(rfa, oracle):
+    from oracle import rfa_warp_oracle as WO
+    w = W.ragged_phantom(dims=(136, 70, 21), spacing=(0.7, 0.9, 1.3), steps=40, dt=0.05)
+    sim = rfa.from_workload(w)
+    sim.step(w.steps)
+    T = sim.get_temperature(0)                               # the fp32 image the warp reads (plus T_a)
+    d = W.breathing_field(w.dims, amp_mm=(2.0, 4.0, 12.0))
+    for scale in (0.0, 0.37, 1.0, -1.0, 40.0):               # 40: far outside the grid -> clamped everywhere
+        got = sim.warp_temperature(0, d, scale)
+        exp = WO.warp_temperature(T, d, np.float32(scale), w.spacing_mm)
+        # tolerance: fp32 interpolation weights (2^-24 relative on a displacement of <= 20 voxels ~ 2e-6 voxel)
+        # times the steepest gradient in the image (53 C per voxel at the needle) + fp32 rounding of the result
+        assert float(np.max(np.abs(got.astype(np.float64) - exp))) <= TOL
+    assert np.array_equal(sim.warp_temperature(0, d, 0.0).view(np.uint32), T.view(np.uint32))
+    import torch
+    dd, od = torch.from_numpy(d).cuda(), torch.empty(T.shape, dtype=torch.float32, device="cuda")
+    sim.warp_temperature(0, dd, 1.0, out=od)                 # device in, device out
+    assert np.array_equal(od.cpu().numpy(), sim.warp_temperature(0, d, 1.0))
+    assert np.array_equal(sim.get_temperature(0).view(np.uint32), T.view(np.uint32))   # state untouched
+    sim.close()
+
+
+def test_warp_full_size_sampled(rfa):
+    """C4 size: sampled voxels against the oracle (it evaluates voxel by voxel), bounds everywhere."""
+    from oracle import rfa_warp_oracle as WO
+    w = W.c4_body(steps=300)
+    sim = rfa.from_workload(w)
+    sim.step(300)
+    T = sim.get_temperature(0)
+    d = W.breathing_field(w.dims)
+    got = sim.warp_temperature(0, d, 0.85)
+    rng = np.random.default_rng(11)
+    mz, my, mx = np.nonzero(w.needles[0].mask)
+    nx, ny, nz = w.dims
+    pick = rng.integers(0, len(mz), 200)
+    near = (np.clip(mx[pick] + rng.integers(-6, 7, 200), 0, nx - 1)
+            + nx * (np.clip(my[pick] + rng.integers(-6, 7, 200), 0, ny - 1)
+                    + ny * np.clip(mz[pick] + rng.integers(-12, 13, 200), 0, nz - 1)))
+    idx = np.unique(np.concatenate([near, rng.integers(0, nx * ny * nz, 4000)]))
+    exp = WO.warp_temperature(T, d, np.float32(0.85), w.spacing_mm, index=idx)
+    assert float(np.max(np.abs(got.ravel()[idx].astype(np.float64) - exp))) <= TOL
+    assert got.min() >= T.min() and got.max() <= T.max()
+    assert float(np.abs(got - T).max()) > 1.0                # the heat zone really moved
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------
 # Full-length configs against the stored oracle results (tests/golden/, written by make_golden.py)
 # ----------------------------------------------------------------------------------------------
 def _golden(name):
