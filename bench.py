@@ -386,6 +386,41 @@ def run_warp(args):
     return 0
 
 
+def run_render(args):
+    """Row f4 (headless view of the heat zone) on the C4 volume: K frames of 512 x 512 pixels, oblique view,
+    0.5 mm steps.  Reported as frame time and trilinear samples per second (no roofline: the kernel is a
+    gather through L2 with fp64 ray arithmetic, neither an HBM stream nor a contraction)."""
+    import torch
+    from paper_1907_05709_b200 import binding, workloads as W
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    w = W.BENCH_CONFIGS[args.config]()
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        sim = binding.from_workload(w, device=dev, stream=stream)
+        sim.step(600)
+        for _ in range(3):
+            tmax, depth = sim.render_zone(0, (1, 2, 3), (0, 1, 0), 512, 512, 0.7, 0.5, 42.5)
+        K = min(args.steps, 20)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            sim.render_zone(0, (1, 2, 3), (0, 1, 0), 512, 512, 0.7, 0.5, 42.5)
+        e1.record(stream)
+        e1.synchronize()
+        ms = float(e0.elapsed_time(e1)) / K
+        sim.close()
+    ext = [n * h for n, h in zip(w.dims, w.spacing_mm)]
+    ns = int(np.floor(np.sqrt(sum(e * e for e in ext)) / 0.5)) + 1
+    print(json.dumps({"metric": "frames/s (heat-zone view, 512x512, host images)", "value": 1e3 / ms, "unit": "frames/s",
+                      "n_gpus": 1, "steps": K, "warmup": 3, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": w.name + " view", "dims": list(w.dims), "image": [512, 512], "step_mm": 0.5,
+                                 "samples_per_ray": ns, "visible_pixels": int((depth >= 0).sum())},
+                      "gsamples_per_s": 512 * 512 * ns / (ms * 1e-3) / 1e9, "roofline": None, "gpu_launches": K}), flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -397,7 +432,7 @@ def main(argv=None):
     ap.add_argument("--fused", type=int, default=0, help="fused time steps per launch, 0 = library default")
     ap.add_argument("--conduction", default="eq12", choices=["eq12", "face"],
                     help="eq12: Eq. 12 as printed (default, the headline); face: conservative div(K grad T), row f1")
-    ap.add_argument("--op", default="step", choices=["step", "warp"],
+    ap.add_argument("--op", default="step", choices=["step", "warp", "render"],
                     help="step: the time-stepping hot path (the headline); warp: the Eq. 14 motion warp (row f3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -408,6 +443,8 @@ def main(argv=None):
         return run_reference(args)
     if args.op == "warp":
         return run_warp(args)
+    if args.op == "render":
+        return run_render(args)
     return run_ours(args)
 
 

@@ -181,6 +181,26 @@ int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_dev, float *
  * Reads the simulation state, does not change it.  Synchronous (waits for the stream). */
 int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp, float scale, float *out);
 
+/* ---- headless view of the heat zone (Figs. 11-12) ----------------
+ * The paper shows the ablation zone as the 42.5 C isotherm in its VR / fluoroscopy views.  No graphics API
+ * is involved here: an orthographic ray-march written as plain CUDA arithmetic into a device (or host) buffer.
+ *   Image plane through the volume centre c (mm), spanned by e1 = normalise(up x dir), e2 = dir x e1 (dir
+ *   normalised first); pixel (px,py) has the offset u = (px-(W-1)/2)*pixel_mm along e1, v likewise along e2.
+ *   Ray: p(m) = c + u e1 + v e2 + (-R + m*step_mm) dir, m = 0 .. floor(2R/step_mm), R = half the volume diagonal.
+ *   A sample counts if it lies inside the box of voxel centres; there T is interpolated trilinearly.
+ *   tmax[py*W+px]  = maximum of T over the ray's samples (t_blood if none lies inside)            [deg C]
+ *   depth[py*W+px] = m*step_mm of the first sample with T >= iso_c, or -1 if there is none        [mm]
+ * Outputs: host or device, W*H floats each; depth may be NULL.  Reads the state only.  Synchronous. */
+typedef struct rfa_view {
+    float dir[3];      /* viewing direction (any non-zero length) */
+    float up[3];       /* not parallel to dir */
+    int width, height; /* pixels */
+    float pixel_mm;    /* pixel spacing on the image plane */
+    float step_mm;     /* sample spacing along the ray */
+    float iso_c;       /* isotherm for the depth image, e.g. 42.5 or 60 (:37) */
+} rfa_view;
+int rfa_render_zone(rfa_sim *s, int scenario, const rfa_view *view, float *tmax, float *depth);
+
 int rfa_synchronize(rfa_sim *s);
 void rfa_destroy(rfa_sim *s);
 const char *rfa_last_error(void);

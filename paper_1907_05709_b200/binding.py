@@ -27,7 +27,7 @@ EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
     "rfa_set_conduction", "rfa_query", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
-    "rfa_warp_temperature",
+    "rfa_warp_temperature", "rfa_render_zone",
     "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
 
@@ -36,6 +36,12 @@ class RfaTissue(ctypes.Structure):
     _fields_ = [("k", ctypes.c_float), ("rho", ctypes.c_float), ("cp", ctypes.c_float),
                 ("wb_cb", ctypes.c_float), ("q_m", ctypes.c_float), ("t_init", ctypes.c_float),
                 ("flags", ctypes.c_uint32)]
+
+
+class RfaView(ctypes.Structure):
+    _fields_ = [("dir", ctypes.c_float * 3), ("up", ctypes.c_float * 3), ("width", ctypes.c_int),
+                ("height", ctypes.c_int), ("pixel_mm", ctypes.c_float), ("step_mm", ctypes.c_float),
+                ("iso_c", ctypes.c_float)]
 
 
 class RfaError(RuntimeError):
@@ -95,6 +101,8 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_current_frame.restype = ctypes.c_int
     lib.rfa_warp_temperature.argtypes = [vp, ctypes.c_int, vp, ctypes.c_float, vp]
     lib.rfa_warp_temperature.restype = ctypes.c_int
+    lib.rfa_render_zone.argtypes = [vp, ctypes.c_int, ctypes.POINTER(RfaView), vp, vp]
+    lib.rfa_render_zone.restype = ctypes.c_int
     lib.rfa_synchronize.argtypes = [vp]
     lib.rfa_synchronize.restype = ctypes.c_int
     lib.rfa_destroy.argtypes = [vp]
@@ -262,6 +270,17 @@ class RfaSim:
             out = np.empty((nz, ny, nx), dtype=np.float32)
         _check(self._lib.rfa_warp_temperature(self._handle, int(scenario), _ptr(d), float(scale), _ptr(out)))
         return out
+
+    def render_zone(self, scenario: int, direction, up, width: int, height: int, pixel_mm: float, step_mm: float,
+                    iso_c: float = 42.5, want_depth: bool = True):
+        """Orthographic ray-march of the heat zone: (tmax image, depth-of-isotherm image), each (height, width)"""
+        v = RfaView((ctypes.c_float * 3)(*[float(x) for x in direction]), (ctypes.c_float * 3)(*[float(x) for x in up]),
+                    int(width), int(height), float(pixel_mm), float(step_mm), float(iso_c))
+        tmax = np.empty((height, width), dtype=np.float32)
+        depth = np.empty((height, width), dtype=np.float32) if want_depth else None
+        _check(self._lib.rfa_render_zone(self._handle, int(scenario), ctypes.byref(v), _ptr(tmax),
+                                         _ptr(depth) if depth is not None else None))
+        return tmax, depth
 
     def synchronize(self):
         _check(self._lib.rfa_synchronize(self._handle))

@@ -648,6 +648,67 @@ extern "C" int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp,
     return RFA_OK;
 }
 
+extern "C" int rfa_render_zone(rfa_sim *s, int scenario, const rfa_view *view, float *tmax, float *depth)
+{
+    int rc = check_sim(s, scenario);
+    if (rc) return rc;
+    if (!view || !tmax) return fail(RFA_E_INVALID, "null argument");
+    if (view->width < 1 || view->height < 1 || (long long)view->width * view->height > (long long)s->nvox / 2 + 4096)
+        return fail(RFA_E_INVALID, "image of %d x %d pixels: need 1 <= W*H <= nx*ny*nz/2", view->width, view->height);
+    if (!(view->pixel_mm > 0.f) || !(view->step_mm > 0.f) || !std::isfinite(view->pixel_mm) || !std::isfinite(view->step_mm) ||
+        !std::isfinite(view->iso_c))
+        return fail(RFA_E_INVALID, "pixel_mm and step_mm must be positive and finite, iso_c finite");
+    RfaRay ray{};
+    double w[3], up[3], n2 = 0;
+    for (int a = 0; a < 3; ++a) {
+        if (!std::isfinite(view->dir[a]) || !std::isfinite(view->up[a])) return fail(RFA_E_INVALID, "dir / up must be finite");
+        w[a] = view->dir[a];
+        up[a] = view->up[a];
+        n2 += w[a] * w[a];
+    }
+    if (!(n2 > 0)) return fail(RFA_E_INVALID, "dir must not be zero");
+    for (int a = 0; a < 3; ++a) w[a] /= std::sqrt(n2);
+    double e1[3] = {up[1] * w[2] - up[2] * w[1], up[2] * w[0] - up[0] * w[2], up[0] * w[1] - up[1] * w[0]};   // up x dir
+    const double l1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    if (!(l1 > 1e-12)) return fail(RFA_E_INVALID, "up must not be parallel to dir");
+    for (int a = 0; a < 3; ++a) e1[a] /= l1;
+    const double e2[3] = {w[1] * e1[2] - w[2] * e1[1], w[2] * e1[0] - w[0] * e1[2], w[0] * e1[1] - w[1] * e1[0]};   // dir x e1
+    const int n[3] = {s->g.nx, s->g.ny, s->g.nz};
+    double diag2 = 0;
+    for (int a = 0; a < 3; ++a) {
+        const double h_mm = s->h_m[a] * 1.0e3;
+        ray.c[a] = 0.5 * n[a] * h_mm;
+        ray.e1[a] = e1[a];
+        ray.e2[a] = e2[a];
+        ray.w[a] = w[a];
+        ray.inv_h[a] = 1.0 / h_mm;
+        diag2 += (n[a] * h_mm) * (n[a] * h_mm);
+    }
+    ray.R = 0.5 * std::sqrt(diag2);
+    ray.pixel = view->pixel_mm;
+    ray.step = view->step_mm;
+    ray.width = view->width;
+    ray.height = view->height;
+    const double ns = std::floor(2.0 * ray.R / ray.step) + 1.0;
+    if (ns > 1.0e6) return fail(RFA_E_INVALID, "step_mm too small: %.0f samples per ray", ns);
+    ray.n_samples = (int)ns;
+    const size_t npix = (size_t)view->width * view->height;
+    // host outputs are staged in the scratch volume (4 bytes per voxel): tmax in its first half, depth in the second
+    const bool tdev = is_device_ptr(tmax), ddev = depth ? is_device_ptr(depth) : true;
+    float *tdst = tdev ? tmax : (float *)s->scratch;
+    float *ddst = depth ? (ddev ? depth : (float *)s->scratch + s->nvox / 2) : nullptr;
+    const float iso_theta = (float)((double)view->iso_c - s->t_blood);
+    cudaError_t e = rfa_launch_render(s->g, scenario, ray, s->theta[s->cur], iso_theta, tdst, ddst, s->stream);
+    s->launches++;
+    if (e != cudaSuccess) return cuda_fail(e, "render kernel");
+    if (!tdev) e = cudaMemcpyAsync(tmax, tdst, npix * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess && depth && !ddev) e = cudaMemcpyAsync(depth, ddst, npix * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "render download");
+    e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "render_zone");
+    return RFA_OK;
+}
+
 extern "C" int rfa_synchronize(rfa_sim *s)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");

@@ -77,6 +77,15 @@ cudaError_t rfa_launch_get_necrosis(const RfaGrid &g, int scenario, const uint8_
                                     cudaStream_t st);
 cudaError_t rfa_launch_warp(const RfaGrid &g, int scenario, const float *theta /*all scenarios*/, const float *disp_dev,
                             float scale, const float inv_h_mm[3], float *out_dev, cudaStream_t st);
+// orthographic camera of rfa_render_zone, set up in fp64 on the host (include/rfa.h: rfa_view)
+struct RfaRay {
+    double c[3], e1[3], e2[3], w[3];   // volume centre (mm), image-plane basis, viewing direction (unit)
+    double inv_h[3];                   // 1 / voxel spacing (1/mm)
+    double R, pixel, step;             // half diagonal, pixel spacing, sample spacing (mm)
+    int width, height, n_samples;
+};
+cudaError_t rfa_launch_render(const RfaGrid &g, int scenario, const RfaRay &ray, const float *theta /*all scenarios*/,
+                              float iso_theta, float *tmax_dev, float *depth_dev /*may be null*/, cudaStream_t st);
 cudaError_t rfa_launch_probe(const RfaGrid &g, int n, const long long *index_dev, const float *theta /*all scenarios*/,
                              float *out_dev, cudaStream_t st);
 cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *state, uint32_t label_held_mask,

@@ -188,6 +188,45 @@ __global__ void rfa_warp_kernel(int nx, int ny, int nz, const float *__restrict_
     }
 }
 
+// headless view of the heat zone (row f4; Figs. 11-12): orthographic ray-march, one thread per pixel.
+// Ray positions are carried in fp64 (a coordinate of ~500 voxels in fp32 would cost 6e-5 voxel = 3e-3 C at the
+// needle's 53 C/voxel gradient); the interpolation itself is fp32 like the warp.
+__global__ void rfa_render_kernel(RfaRay ray, int nx, int ny, int nz, const float *__restrict__ theta, float t_blood,
+                                  float iso_theta, float *__restrict__ tmax, float *__restrict__ depth)
+{
+    const int px = blockIdx.x * blockDim.x + threadIdx.x, py = blockIdx.y * blockDim.y + threadIdx.y;
+    if (px >= ray.width || py >= ray.height) return;
+    const double u = (px - 0.5 * (ray.width - 1)) * ray.pixel, v = (py - 0.5 * (ray.height - 1)) * ray.pixel;
+    double o[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) o[c] = ray.c[c] + u * ray.e1[c] + v * ray.e2[c] - ray.R * ray.w[c];
+    const size_t sy = nx, sz = (size_t)nx * ny;
+    float best = -3.0e38f;
+    int first = -1;
+    for (int m = 0; m < ray.n_samples; ++m) {
+        const double t = m * ray.step;
+        const double qx = (o[0] + t * ray.w[0]) * ray.inv_h[0] - 0.5, qy = (o[1] + t * ray.w[1]) * ray.inv_h[1] - 0.5,
+                     qz = (o[2] + t * ray.w[2]) * ray.inv_h[2] - 0.5;
+        if (qx < 0.0 || qy < 0.0 || qz < 0.0 || qx > nx - 1.0 || qy > ny - 1.0 || qz > nz - 1.0) continue;
+        const int i0 = min((int)qx, max(nx - 2, 0)), j0 = min((int)qy, max(ny - 2, 0)), k0 = min((int)qz, max(nz - 2, 0));
+        const int i1 = min(i0 + 1, nx - 1), j1 = min(j0 + 1, ny - 1), k1 = min(k0 + 1, nz - 1);
+        const float ax = (float)(qx - i0), ay = (float)(qy - j0), az = (float)(qz - k0);
+        const float *z0 = theta + (size_t)k0 * sz, *z1 = theta + (size_t)k1 * sz;
+        const size_t r0 = (size_t)j0 * sy, r1 = (size_t)j1 * sy;
+        const float c000 = __ldg(z0 + r0 + i0), c100 = __ldg(z0 + r0 + i1), c010 = __ldg(z0 + r1 + i0), c110 = __ldg(z0 + r1 + i1);
+        const float c001 = __ldg(z1 + r0 + i0), c101 = __ldg(z1 + r0 + i1), c011 = __ldg(z1 + r1 + i0), c111 = __ldg(z1 + r1 + i1);
+        const float x00 = fmaf(ax, c100 - c000, c000), x10 = fmaf(ax, c110 - c010, c010);
+        const float x01 = fmaf(ax, c101 - c001, c001), x11 = fmaf(ax, c111 - c011, c011);
+        const float y0 = fmaf(ay, x10 - x00, x00), y1 = fmaf(ay, x11 - x01, x01);
+        const float th = fmaf(az, y1 - y0, y0);
+        best = fmaxf(best, th);
+        if (first < 0 && th >= iso_theta) first = m;
+    }
+    const size_t pix = (size_t)py * ray.width + px;
+    tmax[pix] = (best > -1.0e38f ? best : 0.f) + t_blood;
+    if (depth) depth[pix] = first >= 0 ? (float)(first * ray.step) : -1.0f;
+}
+
 // probe read-out (Fig. 6): T at n flat voxel indices of the batched volume
 __global__ void rfa_probe_kernel(int n, const long long *__restrict__ index, const float *__restrict__ theta,
                                  float t_blood, float *__restrict__ out)
@@ -819,6 +858,16 @@ cudaError_t rfa_launch_warp(const RfaGrid &g, int scenario, const float *theta, 
         rfa_warp_kernel<4><<<grid, block, 0, st>>>(g.nx, g.ny, g.nz, th, disp_dev, scale, inv_h_mm[0], inv_h_mm[1], inv_h_mm[2], g.t_blood, out_dev);
     else
         rfa_warp_kernel<1><<<grid, block, 0, st>>>(g.nx, g.ny, g.nz, th, disp_dev, scale, inv_h_mm[0], inv_h_mm[1], inv_h_mm[2], g.t_blood, out_dev);
+    return cudaGetLastError();
+}
+
+cudaError_t rfa_launch_render(const RfaGrid &g, int scenario, const RfaRay &ray, const float *theta, float iso_theta,
+                              float *tmax_dev, float *depth_dev, cudaStream_t st)
+{
+    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    const dim3 block(16, 8, 1), grid((unsigned)((ray.width + 15) / 16), (unsigned)((ray.height + 7) / 8), 1);
+    rfa_render_kernel<<<grid, block, 0, st>>>(ray, g.nx, g.ny, g.nz, theta + (size_t)scenario * nvox, g.t_blood, iso_theta,
+                                              tmax_dev, depth_dev);
     return cudaGetLastError();
 }
 

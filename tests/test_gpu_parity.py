@@ -385,6 +385,34 @@ def test_warp_full_size_sampled(rfa):
 
 
 # ----------------------------------------------------------------------------------------------
+# f4: headless view of the heat zone (orthographic ray-march; Figs. 11-12)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("direction,up", [((0, 0, 1), (0, 1, 0)), ((1, 2, 3), (0, 1, 0)), ((-2, 1, 0.5), (0, 0, 1))])
+def test_render_zone_matches_oracle(rfa, direction, up):
+    from oracle import rfa_render_oracle as RO
+    w = W.c2_phantom(steps=900)
+    sim = rfa.from_workload(w)
+    sim.step(w.steps)
+    T = sim.get_temperature(0)
+    Wp, Hp = 96, 80
+    tmax, depth = sim.render_zone(0, direction, up, Wp, Hp, 1.25, 0.5, iso_c=42.5)
+    etmax, edepth, margin = RO.render_zone(T, w.spacing_mm, direction, up, Wp, Hp, 1.25, 0.5, 42.5, t_blood=w.t_blood)
+    assert float(np.max(np.abs(tmax.astype(np.float64) - etmax))) <= TOL
+    # first-hit decisions: identical wherever no sample of the ray lies within the band of the isotherm
+    clear = margin > BAND
+    assert np.array_equal(depth[clear] >= 0, edepth[clear] >= 0)
+    assert float(np.max(np.abs(depth[clear].astype(np.float64) - edepth[clear]))) <= 1e-4
+    assert int((~clear).sum()) < 0.02 * Wp * Hp and int((edepth >= 0).sum()) > 50      # a zone is visible
+    t2, none = sim.render_zone(0, direction, up, Wp, Hp, 1.25, 0.5, want_depth=False)
+    assert none is None and np.array_equal(t2, tmax)
+    with pytest.raises(rfa.RfaError):
+        sim.render_zone(0, (0, 0, 0), up, Wp, Hp, 1.25, 0.5)
+    with pytest.raises(rfa.RfaError):
+        sim.render_zone(0, up, up, Wp, Hp, 1.25, 0.5)
+    sim.close()
+
+
+# ----------------------------------------------------------------------------------------------
 # Full-length configs against the stored oracle results (tests/golden/, written by make_golden.py)
 # ----------------------------------------------------------------------------------------------
 def _golden(name):
