@@ -770,13 +770,38 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
             }
         };
 
-        for (int i = 0;;) {
-            body(IC<0>{}, i);
-            if (++i >= niter) break;
-            body(IC<1>{}, i);
-            if (++i >= niter) break;
-            body(IC<2>{}, i);
-            if (++i >= niter) break;
+        if constexpr (!CONS) {
+            for (int i = 0;;) {
+                body(IC<0>{}, i);
+                if (++i >= niter) break;
+                body(IC<1>{}, i);
+                if (++i >= niter) break;
+                body(IC<2>{}, i);
+                if (++i >= niter) break;
+            }
+        } else {
+            // The conservative variant carries the face-term code in every mixed / hot path; unrolled three times
+            // it is 185 KB of SASS and stalls on instruction fetch (ncu: no_instruction 1.47 per issue, 380 GVox/s).
+            // One body and an explicit rotation of the plane registers instead: a third of the code, 48 moves more
+            // (446 GVox/s; the same rotation costs the Eq. 12 variant 4.5 %, so that one stays unrolled).
+#pragma unroll 1
+            for (int i = 0; i < niter; ++i) {
+                body(IC<2>{}, i);                          // arrival in slot 2, centre 1, previous 0
+#pragma unroll
+                for (int k = 0; k < S; ++k) {
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        q[k][0][r] = q[k][1][r];
+                        q[k][1][r] = q[k][2][r];
+                    }
+                    nbq[k][0] = nbq[k][1];
+                    nbq[k][1] = nbq[k][2];
+                    hotq[k][0] = hotq[k][1];
+                    hotq[k][1] = hotq[k][2];
+                    rvq[k][0] = rvq[k][1];
+                    rvq[k][1] = rvq[k][2];
+                }
+            }
         }
     }
 }
