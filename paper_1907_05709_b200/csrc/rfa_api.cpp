@@ -58,7 +58,7 @@ struct rfa_sim {
     int kernel = RFA_KERNEL_AUTO;
     int fused = 3;
     RfaTbPlan plans[5]{};                // index = fused steps 1..4
-    int resident[5]{};
+    int resident[5][RFA_N_SHAPES]{};
     long long launches = 0;
     long long *probes = nullptr;         // device, n_probes flat voxel indices (library-owned)
     int n_probes = 0;
@@ -169,13 +169,15 @@ static void build_table(const rfa_sim *s, double q_power, RfaTableHost &out)
 // ------------------------------------------------------------------------------------------------
 // plan of the blocked kernel (host only)
 // ------------------------------------------------------------------------------------------------
-RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int resident_ctas)
+static RfaTbPlan plan_shape(int nx, int ny, int nz, int batch, int S, int shape, int resident_ctas, double &cost_out)
 {
     RfaTbPlan p{};
-    p.fused = fused;
-    const int S = fused;
-    if (S < 1 || S > 4 || nx < 4 || (nx % 4) != 0 || ny < S || nz < S || batch < 1 || resident_ctas < 1) return p;
-    const int BX = 4 * RFA_TB_SHAPE[S].tx, BY = RFA_TB_SHAPE[S].ry * RFA_TB_SHAPE[S].ty;
+    p.fused = S;
+    p.shape = shape;
+    cost_out = 1e300;
+    if (resident_ctas < 1) return p;
+    const int BX = 4 * RFA_TB_SHAPE[shape][S].tx, BY = RFA_TB_SHAPE[shape][S].ry * RFA_TB_SHAPE[shape][S].ty;
+    if (BY <= 2 * S) return p;
     p.tiles_x = nx <= BX ? 1 : (nx - 8 + (BX - 8) - 1) / (BX - 8);
     p.tiles_y = (ny + (BY - 2 * S) - 1) / (BY - 2 * S);
     const long long per_z = (long long)p.tiles_x * p.tiles_y * batch;
@@ -198,14 +200,36 @@ RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int res
     p.n_items = (int)items;
     p.grid = (int)std::min<long long>(items, resident_ctas);
     p.ok = 1;
+    cost_out = best;
     return p;
+}
+
+RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const int resident_ctas[RFA_N_SHAPES])
+{
+    RfaTbPlan best{};
+    best.fused = fused;
+    const int S = fused;
+    if (S < 1 || S > 4 || nx < 4 || (nx % 4) != 0 || ny < S || nz < S || batch < 1 || !resident_ctas) return best;
+    double best_cost = 1e300;
+    for (int shape = 0; shape < RFA_N_SHAPES; ++shape) {
+        double cost;
+        RfaTbPlan p = plan_shape(nx, ny, nz, batch, S, shape, resident_ctas[shape], cost);
+        // every CTA has 256 threads and 8 voxels per thread and plane, so plane iterations compare directly;
+        // the wide shape must win by 5 % (its y halo costs more redundant rows per useful one)
+        if (p.ok && cost < best_cost * (shape == 0 ? 1.0 : 0.95)) {
+            best = p;
+            best_cost = cost;
+        }
+    }
+    return best;
 }
 
 // exported for the CPU unit tests of the planner (no GPU needed)
 extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resident_ctas, int out[9])
 {
     if (!dims || !out) return RFA_E_INVALID;
-    RfaTbPlan p = rfa_plan_blocked(dims[0], dims[1], dims[2], batch, fused, resident_ctas);
+    const int res[RFA_N_SHAPES] = {resident_ctas, resident_ctas};
+    RfaTbPlan p = rfa_plan_blocked(dims[0], dims[1], dims[2], batch, fused, res);
     out[0] = p.ok;
     out[1] = p.tiles_x;
     out[2] = p.tiles_y;
@@ -213,8 +237,8 @@ extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resid
     out[4] = p.zchunk;
     out[5] = p.n_items;
     out[6] = p.grid;
-    out[7] = p.ok ? 4 * RFA_TB_SHAPE[fused].tx : 0;
-    out[8] = p.ok ? RFA_TB_SHAPE[fused].ry * RFA_TB_SHAPE[fused].ty : 0;
+    out[7] = p.ok ? 4 * RFA_TB_SHAPE[p.shape][fused].tx : 0;
+    out[8] = p.ok ? RFA_TB_SHAPE[p.shape][fused].ry * RFA_TB_SHAPE[p.shape][fused].ty : 0;
     return RFA_OK;
 }
 
@@ -252,7 +276,7 @@ static int upload_table(rfa_sim *s, int scenario)
 static void make_plans(rfa_sim *s)
 {
     for (int f = 1; f <= 4; ++f) {
-        s->resident[f] = rfa_blocked_resident_ctas(f);
+        for (int sh = 0; sh < RFA_N_SHAPES; ++sh) s->resident[f][sh] = rfa_blocked_resident_ctas(f, sh);
         s->plans[f] = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, s->resident[f]);
     }
 }

@@ -17,6 +17,7 @@ struct RfaGrid {
 // Plan of the temporally blocked kernel for one launch geometry.
 struct RfaTbPlan {
     int fused;                 // S: time steps per launch, 1..4
+    int shape;                 // index into RFA_TB_SHAPE
     int tiles_x, tiles_y;      // xy tiling
     int nzc, zchunk;           // z chunks
     int n_items;               // batch * nzc * tiles_y * tiles_x
@@ -52,14 +53,25 @@ struct RfaTbShape {
 #define RFA_S4_RY 2
 #define RFA_S4_MINB 2
 #endif
-constexpr RfaTbShape RFA_TB_SHAPE[5] = {{0, 0, 0, 0},
-                                        {RFA_TX, RFA_TY, RFA_S1_RY, RFA_S1_MINB},
-                                        {RFA_TX, RFA_TY, RFA_S2_RY, RFA_S2_MINB},
-                                        {RFA_TX, RFA_TY, RFA_S3_RY, RFA_S3_MINB},
-                                        {RFA_TX, RFA_TY, RFA_S4_RY, RFA_S4_MINB}};
+// Two thread arrangements of the same 256-thread CTA, chosen per grid by the planner (fewest plane iterations):
+//   shape 0  16 x 16 threads: tile 64 x 32  -- few y halo rows; the default on wide grids
+//   shape 1  32 x  8 threads: tile 128 x 16 -- a whole 128-voxel row per tile (no x halo at all for nx <= 128:
+//            the 128^3 planning-sweep volumes run 1.3x faster with it)
+#define RFA_N_SHAPES 2
+constexpr RfaTbShape RFA_TB_SHAPE[RFA_N_SHAPES][5] = {{{0, 0, 0, 0},
+                                                       {RFA_TX, RFA_TY, RFA_S1_RY, RFA_S1_MINB},
+                                                       {RFA_TX, RFA_TY, RFA_S2_RY, RFA_S2_MINB},
+                                                       {RFA_TX, RFA_TY, RFA_S3_RY, RFA_S3_MINB},
+                                                       {RFA_TX, RFA_TY, RFA_S4_RY, RFA_S4_MINB}},
+                                                      {{0, 0, 0, 0},
+                                                       {2 * RFA_TX, RFA_TY / 2, RFA_S1_RY, RFA_S1_MINB},
+                                                       {2 * RFA_TX, RFA_TY / 2, RFA_S2_RY, RFA_S2_MINB},
+                                                       {2 * RFA_TX, RFA_TY / 2, RFA_S3_RY, RFA_S3_MINB},
+                                                       {2 * RFA_TX, RFA_TY / 2, RFA_S4_RY, RFA_S4_MINB}}};
 
 // host-only planning (no CUDA calls): implemented in rfa_api.cpp, unit-tested on CPU
-RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, int resident_ctas);
+// resident_ctas: co-resident CTAs per shape (0 = this shape cannot run)
+RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const int resident_ctas[RFA_N_SHAPES]);
 
 // launchers (rfa_kernels.cu).  All asynchronous on `st`; return cudaGetLastError().
 cudaError_t rfa_launch_table(const RfaTableHost &tbl, float *dst, cudaStream_t st);
@@ -97,4 +109,4 @@ cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const fl
                                const void *rin, void *rout, uint8_t *state, const float *tables, const float *kap,
                                cudaStream_t st);
 // resident CTAs of the blocked kernel on the current device for `fused` steps (occupancy * SM count)
-int rfa_blocked_resident_ctas(int fused);
+int rfa_blocked_resident_ctas(int fused, int shape);

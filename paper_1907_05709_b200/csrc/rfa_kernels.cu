@@ -922,17 +922,17 @@ cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, co
     return cudaGetLastError();
 }
 
-template <int S, bool CONS>
+template <int S, bool CONS, int SHAPE>
 struct TbKernel {
-    static constexpr RfaTbShape sh = RFA_TB_SHAPE[S];
+    static constexpr RfaTbShape sh = RFA_TB_SHAPE[SHAPE][S];
     using C = TbCfg<S, sh.tx, sh.ty, sh.ry, CONS>;
     static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb, CONS>; }
 };
 
-template <int S, bool CONS>
+template <int S, bool CONS, int SHAPE>
 static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_t st)
 {
-    using K = TbKernel<S, CONS>;
+    using K = TbKernel<S, CONS, SHAPE>;
     auto kern = K::get();
     static bool attr_set = false;
     if (!attr_set) {
@@ -945,9 +945,10 @@ static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_
 }
 
 template <int S>
-static cudaError_t launch_blocked_s(const RfaTbParams &p, int grid, cudaStream_t st)
+static cudaError_t launch_blocked_s(const RfaTbParams &p, int shape, int grid, cudaStream_t st)
 {
-    return p.kap != nullptr ? launch_blocked_sc<S, true>(p, grid, st) : launch_blocked_sc<S, false>(p, grid, st);
+    if (shape == 0) return p.kap != nullptr ? launch_blocked_sc<S, true, 0>(p, grid, st) : launch_blocked_sc<S, false, 0>(p, grid, st);
+    return p.kap != nullptr ? launch_blocked_sc<S, true, 1>(p, grid, st) : launch_blocked_sc<S, false, 1>(p, grid, st);
 }
 
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
@@ -977,18 +978,18 @@ cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const fl
     p.zchunk = plan.zchunk;
     p.n_items = plan.n_items;
     switch (plan.fused) {
-    case 1: return launch_blocked_s<1>(p, plan.grid, st);
-    case 2: return launch_blocked_s<2>(p, plan.grid, st);
-    case 3: return launch_blocked_s<3>(p, plan.grid, st);
-    case 4: return launch_blocked_s<4>(p, plan.grid, st);
+    case 1: return launch_blocked_s<1>(p, plan.shape, plan.grid, st);
+    case 2: return launch_blocked_s<2>(p, plan.shape, plan.grid, st);
+    case 3: return launch_blocked_s<3>(p, plan.shape, plan.grid, st);
+    case 4: return launch_blocked_s<4>(p, plan.shape, plan.grid, st);
     default: return cudaErrorInvalidValue;
     }
 }
 
-template <int S>
+template <int S, int SHAPE>
 static int resident_s()
 {
-    using K = TbKernel<S, true>;            // the conservative variant needs the larger state ring: plan for it
+    using K = TbKernel<S, true, SHAPE>;     // the conservative variant needs the larger state ring: plan for it
     auto kern = K::get();
     int dev = 0, sms = 0, occ = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;
@@ -1003,13 +1004,22 @@ static int resident_s()
     return sms * occ;
 }
 
-int rfa_blocked_resident_ctas(int fused)
+int rfa_blocked_resident_ctas(int fused, int shape)
 {
+    if (shape == 0) {
+        switch (fused) {
+        case 1: return resident_s<1, 0>();
+        case 2: return resident_s<2, 0>();
+        case 3: return resident_s<3, 0>();
+        case 4: return resident_s<4, 0>();
+        default: return 0;
+        }
+    }
     switch (fused) {
-    case 1: return resident_s<1>();
-    case 2: return resident_s<2>();
-    case 3: return resident_s<3>();
-    case 4: return resident_s<4>();
+    case 1: return resident_s<1, 1>();
+    case 2: return resident_s<2, 1>();
+    case 3: return resident_s<3, 1>();
+    case 4: return resident_s<4, 1>();
     default: return 0;
     }
 }

@@ -120,6 +120,15 @@ def test_blocked_plan_covers_the_grid(lib, dims, batch, fused):
     assert p["ctas"] == min(p["work_items"], 148)
 
 
+def test_planner_picks_the_tile_shape_by_grid(lib):
+    """Two arrangements of the 256-thread CTA: 64 x 32 tiles on wide grids, whole 128-voxel rows (128 x 16 tiles) where
+    that needs fewer plane iterations (the 128^3 planning-sweep volumes)."""
+    assert binding.plan_query((512, 512, 256), 1, 3, 296)["bx"] == 64
+    assert binding.plan_query((256, 256, 256), 1, 3, 296)["bx"] == 64
+    p = binding.plan_query((128, 128, 128), 64, 3, 296)
+    assert (p["bx"], p["by"], p["tiles_x"]) == (128, 16, 1)
+
+
 def test_blocked_plan_rejects_unsupported_grids(lib):
     assert binding.plan_query((45, 38, 29), 1, 2, 148)["ok"] == 0      # nx % 4 != 0 -> plain kernel
     assert binding.plan_query((44, 38, 1), 1, 2, 148)["ok"] == 0       # nz < fused steps
