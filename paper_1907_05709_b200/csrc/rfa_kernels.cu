@@ -346,6 +346,7 @@ struct RfaTbParams {
     int nx4;
     float wx, wy, wz, thr;
     int tiles_x, tiles_y, nzc, zchunk, n_items;
+    int held_copy;                    // kernel variant: warps of held voxels only copy their rows (HELDCOPY)
 };
 
 constexpr int rfa_pow2_at_least(int n) { return n <= 1 ? 1 : 2 * rfa_pow2_at_least((n + 1) / 2); }
@@ -441,7 +442,7 @@ struct IC {
     static constexpr int value = I;
 };
 
-template <int S, int TX, int TY, int RY, int MINB, bool CONS>
+template <int S, int TX, int TY, int RY, int MINB, bool CONS, bool HELDCOPY>
 __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbParams P)
 {
     using C = TbCfg<S, TX, TY, RY, CONS>;
@@ -670,13 +671,26 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                         const unsigned e = sw[k][0] & RFA_ST_INDEX;
                         const float a = tab[e], nk = tab[RFA_TABLE_N + e], qa = tab[2 * RFA_TABLE_N + e];
                         const u64 a2 = pk(a, a), n2 = pk(nk, nk), q2 = pk(qa, qa);
+                        if (HELDCOPY && __all_sync(0xffffffffu, a == 0.f)) {
+                            // every voxel of the warp is held (a = 0: exterior, vessel, Dirichlet needle): Alg. 1's
+                            // else-branch, "copy the input voxel".  theta + fma(0, g, +0) = theta + (+0)
+                            // for any finite g, so the bracket need not be evaluated; bit-identical to the full path
 #pragma unroll
-                        for (int r = 0; r < RY; ++r) {
-                            u64 t01, t23, g01, g23;
-                            bracket_row(r, n2, n2, q2, q2, t01, t23, g01, g23, false);
-                            upk(add2(t01, fma2(a2, g01, zero2)), o[r].x, o[r].y);
-                            upk(add2(t23, fma2(a2, g23, zero2)), o[r].z, o[r].w);
-                            mx = max_abs4(o[r], mx);
+                            for (int r = 0; r < RY; ++r) {
+                                const float4 c = q[k][CE][r];
+                                upk(add2(pk(c.x, c.y), zero2), o[r].x, o[r].y);
+                                upk(add2(pk(c.z, c.w), zero2), o[r].z, o[r].w);
+                                mx = max_abs4(o[r], mx);
+                            }
+                        } else {
+#pragma unroll
+                            for (int r = 0; r < RY; ++r) {
+                                u64 t01, t23, g01, g23;
+                                bracket_row(r, n2, n2, q2, q2, t01, t23, g01, g23, false);
+                                upk(add2(t01, fma2(a2, g01, zero2)), o[r].x, o[r].y);
+                                upk(add2(t23, fma2(a2, g23, zero2)), o[r].z, o[r].w);
+                                mx = max_abs4(o[r], mx);
+                            }
                         }
                     } else {
 #pragma unroll
@@ -922,17 +936,17 @@ cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, co
     return cudaGetLastError();
 }
 
-template <int S, bool CONS, int SHAPE>
+template <int S, bool CONS, int SHAPE, bool HC = false>
 struct TbKernel {
     static constexpr RfaTbShape sh = RFA_TB_SHAPE[SHAPE][S];
     using C = TbCfg<S, sh.tx, sh.ty, sh.ry, CONS>;
-    static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb, CONS>; }
+    static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb, CONS, HC>; }
 };
 
-template <int S, bool CONS, int SHAPE>
+template <int S, bool CONS, int SHAPE, bool HC>
 static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_t st)
 {
-    using K = TbKernel<S, CONS, SHAPE>;
+    using K = TbKernel<S, CONS, SHAPE, HC>;
     auto kern = K::get();
     static bool attr_set = false;
     if (!attr_set) {
@@ -947,8 +961,13 @@ static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_
 template <int S>
 static cudaError_t launch_blocked_s(const RfaTbParams &p, int shape, int grid, cudaStream_t st)
 {
-    if (shape == 0) return p.kap != nullptr ? launch_blocked_sc<S, true, 0>(p, grid, st) : launch_blocked_sc<S, false, 0>(p, grid, st);
-    return p.kap != nullptr ? launch_blocked_sc<S, true, 1>(p, grid, st) : launch_blocked_sc<S, false, 1>(p, grid, st);
+    const bool cons = p.kap != nullptr, hc = p.held_copy != 0;
+    if (shape == 0) {
+        if (cons) return hc ? launch_blocked_sc<S, true, 0, true>(p, grid, st) : launch_blocked_sc<S, true, 0, false>(p, grid, st);
+        return hc ? launch_blocked_sc<S, false, 0, true>(p, grid, st) : launch_blocked_sc<S, false, 0, false>(p, grid, st);
+    }
+    if (cons) return hc ? launch_blocked_sc<S, true, 1, true>(p, grid, st) : launch_blocked_sc<S, true, 1, false>(p, grid, st);
+    return hc ? launch_blocked_sc<S, false, 1, true>(p, grid, st) : launch_blocked_sc<S, false, 1, false>(p, grid, st);
 }
 
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
@@ -977,6 +996,7 @@ cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const fl
     p.nzc = plan.nzc;
     p.zchunk = plan.zchunk;
     p.n_items = plan.n_items;
+    p.held_copy = g.held_copy;
     switch (plan.fused) {
     case 1: return launch_blocked_s<1>(p, plan.shape, plan.grid, st);
     case 2: return launch_blocked_s<2>(p, plan.shape, plan.grid, st);
