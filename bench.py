@@ -261,6 +261,7 @@ def run_ours(args):
             dist.barrier()
         ms_local = float(e0.elapsed_time(e1))
         q1 = sim.query()
+        variant = sim.query_variant()
         necro_all, necro_tissue = sim.necrotic_voxels(0)
         tmax = float(sim.get_temperature(0).max())
         sim.close()
@@ -334,7 +335,7 @@ def run_ours(args):
                        "l2": "inputs larger than L2 (2 x %d MiB fields + %d MiB state vs 126 MB L2)" % (
                            nvox_all * 4 >> 20, nvox_all >> 20) if nvox_all * 9 > 126e6 * 2 else
                              "working set fits L2 (reported, not held to the HBM bar)",
-                       "kernel": roofline["kernel"], "conduction": args.conduction},
+                       "kernel": roofline["kernel"], "conduction": args.conduction, "variant": variant},
             "sim_steps_per_s": K / (ms * 1e-3) * (1 if world == 1 else world),
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
             "clocks": clk.summary(),

@@ -141,6 +141,13 @@ int rfa_set_conduction(rfa_sim *s, int mode);
 /* Introspection: fused steps in use, kernel in use, number of kernel launches issued so far by this simulation. */
 int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launches);
 
+/* The variant rfa_step launches for this simulation:
+ * out = { fused_steps, tile_bx, tile_by, ctas_launched, held_copy, conduction }.  held_copy = 1: the kernel variant in
+ * which warps whose voxels are all held copy their rows instead of evaluating the bracket (Alg. 1's else-branch,
+ * PAPER.md:313; bit-identical), chosen at rfa_create when at least 1/8 of the volume carries a held label
+ * (environment variable RFA_HELD_COPY=0/1 overrides, for A/B measurements).  Zeros for the plain kernel. */
+int rfa_query_variant(rfa_sim *s, int out[6]);
+
 /* Host-only view of the blocked kernel's launch plan for a grid (no GPU needed; used by the unit tests
  * and the bench report).  resident_ctas = CTAs that can be co-resident (SM count x occupancy).
  * out = { ok, tiles_x, tiles_y, z_chunks, planes_per_chunk, work_items, ctas_launched, tile_bx, tile_by }. */

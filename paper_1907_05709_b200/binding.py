@@ -26,7 +26,7 @@ COND_EQ12, COND_FACE = 0, 1
 EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
-    "rfa_set_conduction", "rfa_query", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
+    "rfa_set_conduction", "rfa_query", "rfa_query_variant", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
     "rfa_warp_temperature", "rfa_render_zone",
     "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
@@ -91,6 +91,8 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_set_conduction.restype = ctypes.c_int
     lib.rfa_query.argtypes = [vp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int64)]
     lib.rfa_query.restype = ctypes.c_int
+    lib.rfa_query_variant.argtypes = [vp, ctypes.POINTER(ctypes.c_int)]
+    lib.rfa_query_variant.restype = ctypes.c_int
     lib.rfa_plan_query.argtypes = [i3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
     lib.rfa_plan_query.restype = ctypes.c_int
     lib.rfa_set_probes.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int64)]
@@ -242,6 +244,11 @@ class RfaSim:
         k, f, n = ctypes.c_int(), ctypes.c_int(), ctypes.c_int64()
         _check(self._lib.rfa_query(self._handle, ctypes.byref(k), ctypes.byref(f), ctypes.byref(n)))
         return {"kernel": int(k.value), "fused_steps": int(f.value), "kernel_launches": int(n.value)}
+
+    def query_variant(self) -> dict:
+        out = (ctypes.c_int * 6)()
+        _check(self._lib.rfa_query_variant(self._handle, out))
+        return dict(zip(["fused_steps", "tile_bx", "tile_by", "ctas", "held_copy", "conduction"], [int(x) for x in out]))
 
     def set_probes(self, index):
         idx = np.ascontiguousarray(index, dtype=np.int64).reshape(-1)

@@ -574,6 +574,20 @@ static int advance(rfa_sim *s, int n)
     return RFA_OK;
 }
 
+extern "C" int rfa_query_variant(rfa_sim *s, int out[6])
+{
+    if (!s || !out) return fail(RFA_E_INVALID, "null argument");
+    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
+    const RfaTbPlan &p = s->plans[s->fused];
+    out[0] = blocked ? s->fused : 1;
+    out[1] = blocked ? 4 * RFA_TB_SHAPE[p.shape][s->fused].tx : 0;
+    out[2] = blocked ? RFA_TB_SHAPE[p.shape][s->fused].ry * RFA_TB_SHAPE[p.shape][s->fused].ty : 0;
+    out[3] = blocked ? p.grid : 0;
+    out[4] = blocked ? s->g.held_copy : 0;
+    out[5] = s->conduction;
+    return RFA_OK;
+}
+
 extern "C" int rfa_step(rfa_sim *s, int n)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");

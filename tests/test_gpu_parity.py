@@ -232,6 +232,26 @@ def test_monotone_and_bounded_on_gpu(rfa):
     sim.close()
 
 
+def test_held_copy_variant_is_bit_identical(rfa, monkeypatch):
+    """Warps of held voxels only copy their rows (Alg. 1's else-branch): same bits as evaluating the bracket."""
+    w = W.ragged_phantom(dims=(136, 70, 21), spacing=(0.7, 0.9, 1.3), steps=33, dt=0.05)
+    res = {}
+    for hc in ("0", "1"):
+        monkeypatch.setenv("RFA_HELD_COPY", hc)
+        sim = rfa.from_workload(w)
+        sim.configure(rfa.KERNEL_BLOCKED, 3)
+        assert sim.query_variant()["held_copy"] == int(hc) and sim.query_variant()["tile_bx"] in (64, 128)
+        sim.step(w.steps)
+        res[hc] = (sim.get_temperature(0), sim.get_necrosis(0))
+        sim.close()
+    assert np.array_equal(res["0"][0].view(np.uint32), res["1"][0].view(np.uint32))
+    assert np.array_equal(res["0"][1], res["1"][1])
+    monkeypatch.delenv("RFA_HELD_COPY")
+    sim = rfa.from_workload(W.c1_cube())                      # no held label at all: the plain variant is chosen
+    assert sim.query_variant()["held_copy"] == 0
+    sim.close()
+
+
 # ----------------------------------------------------------------------------------------------
 # f1: conservative conduction (harmonic-mean face conductivities, DESIGN.md R-28)
 # ----------------------------------------------------------------------------------------------
