@@ -337,6 +337,10 @@ def run_ours(args):
                              "working set fits L2 (reported, not held to the HBM bar)",
                        "kernel": roofline["kernel"], "conduction": args.conduction, "variant": variant},
             "sim_steps_per_s": K / (ms * 1e-3) * (1 if world == 1 else world),
+            # BASELINE.json's "% of B200 HBM roofline": voxel-updates/s x 8 B (one read + one write of the fp32 field per
+            # time step, north_star) over the measured copy bandwidth; roofline.frac below uses the bytes the kernel
+            # must really move (11 B per voxel per launch of S fused steps), which temporal blocking shrinks on purpose
+            "hbm_roofline_equiv_frac": roofline["equiv_8B_frac"],
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
             "clocks": clk.summary(),
             "check": {"t_max_c": tmax, "necrotic_voxels": necro_all, "necrotic_tissue_voxels": necro_tissue},
