@@ -132,4 +132,6 @@ def test_planner_picks_the_tile_shape_by_grid(lib):
 def test_blocked_plan_rejects_unsupported_grids(lib):
     assert binding.plan_query((45, 38, 29), 1, 2, 148)["ok"] == 0      # nx % 4 != 0 -> plain kernel
     assert binding.plan_query((44, 38, 1), 1, 2, 148)["ok"] == 0       # nz < fused steps
+    assert binding.plan_query((4096, 4096, 512), 1, 3, 296)["ok"] == 0  # 8.6e9 voxels: beyond 32-bit float4 offsets
+    assert binding.plan_query((2048, 2048, 1024), 1, 3, 296)["ok"] == 1
     assert binding.plan_query((44, 38, 29), 1, 5, 148)["ok"] == 0
