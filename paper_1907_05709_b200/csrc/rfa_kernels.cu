@@ -603,8 +603,12 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 // publish first/last row of the arriving level-k plane (it is the centre plane next iteration)
                 exch[((k * 2 + par_w) * 2 + 0) * NT + tid] = q[k][PH][0];
                 exch[((k * 2 + par_w) * 2 + 1) * NT + tid] = q[k][PH][RY - 1];
-                const float4 above = exch[((k * 2 + par_r) * 2 + 1) * NT + up_tid];
-                const float4 below = exch[((k * 2 + par_r) * 2 + 0) * NT + dn_tid];
+                // rows of the neighbouring threads (centre plane): fetched only by the paths that evaluate the bracket
+                float4 above, below;
+                auto load_rows = [&]() {
+                    above = exch[((k * 2 + par_r) * 2 + 1) * NT + up_tid];
+                    below = exch[((k * 2 + par_r) * 2 + 0) * NT + dn_tid];
+                };
                 float mx = 0.f;                            // max |theta'| over this thread's voxels
                 float4 o[RY];
 
@@ -683,6 +687,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                                 mx = max_abs4(o[r], mx);
                             }
                         } else {
+                            load_rows();
 #pragma unroll
                             for (int r = 0; r < RY; ++r) {
                                 u64 t01, t23, g01, g23;
@@ -693,6 +698,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                             }
                         }
                     } else {
+                        load_rows();
 #pragma unroll
                         for (int r = 0; r < RY; ++r) {
                             u64 a01, a23, n01, n23, q01, q23, t01, t23, g01, g23;
@@ -711,6 +717,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                     // rfa_advance() in full, two voxels per instruction (o - t and d - bv as exact-product FMAs)
                     const u64 neg1 = pk(-1.0f, -1.0f), mg = pk(RFA_COMP_MAGIC, RFA_COMP_MAGIC), nmg = pk(-RFA_COMP_MAGIC, -RFA_COMP_MAGIC);
                     const unsigned plc = (unsigned)rfa_reflect(z0 - S + i - 1, P.nz) * plane4;   // level-0 centre plane
+                    load_rows();
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
                         float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
