@@ -42,7 +42,7 @@ METRIC = "GVoxel-updates/s"
 STATE_BYTES_PER_VOXEL_PASS = 11.0    # 4 B theta read + 4 B theta write + 1 B state read + 2 B residual write
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the one
 # `ncu --set full` capture committed under profiles/ (r1_blocked_s3_ncu_full.md); keyed by (config, fused steps)
-NCU_TRAFFIC_BYTES = {("C4", 3): 714.8e6}
+NCU_TRAFFIC_BYTES = {("C4", 3): 729.5e6}
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
