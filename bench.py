@@ -372,7 +372,7 @@ def run_warp(args):
         with ClockSampler(dev.index or 0) as clk:
             e0.record(stream)
             for _ in range(K):
-                sim.warp_temperature(0, d, 0.85, out=out)
+                sim.warp_temperature(0, d, 0.85, out=out)       # device in / device out: asynchronous
             e1.record(stream)
             e1.synchronize()
         ms = float(e0.elapsed_time(e1))

@@ -185,7 +185,8 @@ int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_dev, float *
  *   out    host or device, nx*ny*nz floats, deg C:
  *          out[v] = trilinear interpolation of the current temperature image of `scenario` at the position
  *          (voxel centre of v) + scale*disp[v], sample positions clamped to the volume of voxel centres.
- * Reads the simulation state, does not change it.  Synchronous (waits for the stream). */
+ * Reads the simulation state, does not change it.  Waits for the stream unless both `disp` and `out` are device
+ * memory (then it is asynchronous like rfa_step; rfa_synchronize orders the caller's read of `out`). */
 int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp, float scale, float *out);
 
 /* ---- headless view of the heat zone (Figs. 11-12) ----------------

@@ -701,7 +701,8 @@ extern "C" int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp,
     e = rfa_launch_warp(s->g, scenario, s->theta[s->cur], ddev, scale, inv_h, dst, s->stream);
     s->launches++;
     if (e == cudaSuccess && !dev) e = cudaMemcpyAsync(out, dst, nvox * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
-    cudaError_t e2 = cudaStreamSynchronize(s->stream);
+    // device field in, device image out: nothing of the caller's is touched after the launch -> asynchronous
+    cudaError_t e2 = (tmp != nullptr || !dev) ? cudaStreamSynchronize(s->stream) : cudaSuccess;
     if (tmp) cudaFree(tmp);
     if (e != cudaSuccess) return cuda_fail(e, "warp kernel");
     if (e2 != cudaSuccess) return cuda_fail(e2, "warp_temperature");
