@@ -165,7 +165,17 @@ def cpu_baseline(w, budget_s=15.0, conservative=False):
     n = int(max(1, min(5000, budget_s / max(secs1, 1e-3))))
     secs, nv, thr, _ = oracle_time(w, n, 0, w.dims[2], conservative)
     gv = nv * n / secs / 1e9
-    return {"value": gv, "unit": METRIC, "cores": thr, "kind": "oracle",
+    # the same oracle on ONE thread: a few steps, ~5 s
+    from oracle import rfa_oracle
+    rfa_oracle.set_num_threads(1)
+    try:
+        s1, nv1, _, _ = oracle_time(w, 1, 0, w.dims[2], conservative)
+        n1 = int(max(1, min(50, 5.0 / max(s1, 1e-3))))
+        s1, nv1, _, _ = oracle_time(w, n1, 0, w.dims[2], conservative)
+        single = {"value": nv1 * n1 / s1 / 1e9, "unit": METRIC, "cores": 1, "steps": n1}
+    finally:
+        rfa_oracle.set_num_threads(thr)
+    return {"value": gv, "unit": METRIC, "cores": thr, "kind": "oracle", "single_thread": single,
             "sample": f"{n} time steps of the full {w.dims[0]}x{w.dims[1]}x{w.dims[2]} {w.name} volume, fp64, "
                       f"OpenMP over z ({secs:.1f} s)",
             "steps_per_s": n / secs}
