@@ -246,6 +246,30 @@ def test_held_copy_variant_is_bit_identical(rfa, monkeypatch):
         sim.close()
     assert np.array_equal(res["0"][0].view(np.uint32), res["1"][0].view(np.uint32))
     assert np.array_equal(res["0"][1], res["1"][1])
+    # a body in air: whole tile planes are held (the CTA-wide shortcut), others are cut by the body surface
+    nx, ny, nz = 200, 136, 24
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    rr = ((i - 120) / 60.0) ** 2 + ((j - 70) / 40.0) ** 2 + ((k - 11) / 9.0) ** 2
+    lab = np.full((nz, ny, nx), W.EXTERIOR, np.uint8)
+    lab[rr < 1.0] = W.FAT
+    lab[rr < 0.5] = W.LIVER
+    lab[(rr < 0.5) & (np.abs(j - 62) < 3) & (np.abs(k - 9) < 3)] = W.VESSEL
+    mask = np.zeros_like(lab)
+    mask[11, 70, 108:132] = 1
+    body = {}
+    for hc in ("0", "1"):
+        monkeypatch.setenv("RFA_HELD_COPY", hc)
+        for fused in (3, 2):
+            sim = rfa.RfaSim((nx, ny, nz), (0.9, 0.9, 1.2), lab, W.tissue_table(), 37.0, 0.05)
+            sim.configure(rfa.KERNEL_BLOCKED, fused)
+            sim.set_needle(0, mask, rfa.SRC_DIRICHLET, 90.0)
+            sim.step(40)
+            body[(hc, fused)] = (sim.get_temperature(0), sim.get_necrosis(0))
+            sim.close()
+    ref = body[("0", 3)]
+    assert float(ref[0].max()) == 90.0 and float(ref[0][11, 71, 110]) > 37.5
+    for key, (T, N) in body.items():
+        assert np.array_equal(T.view(np.uint32), ref[0].view(np.uint32)) and np.array_equal(N, ref[1]), key
     monkeypatch.delenv("RFA_HELD_COPY")
     sim = rfa.from_workload(W.c1_cube())                      # no held label at all: the plain variant is chosen
     assert sim.query_variant()["held_copy"] == 0
