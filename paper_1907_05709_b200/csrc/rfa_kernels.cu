@@ -131,25 +131,26 @@ __global__ void rfa_get_necrosis_kernel(size_t nvox, const uint8_t *__restrict__
 // breathing-motion warp, Eq. 14: out[v] = T(x_v + scale * u[v]), trilinear, clamped (row f3).
 // The displacement is split into integer and fractional voxels BEFORE the voxel index is added, so the
 // interpolation weights keep the full fp32 resolution of the (small) displacement, not of the coordinate.
+// one axis of the sample position: the displacement d (in voxels) is clamped so that base + d stays inside
+// [0, n-1] (bounds exact in fp32: small integers), then split into cell index and weight.  d keeps its own fp32
+// resolution: it is never added to the coordinate in floating point.
+__device__ __forceinline__ void rfa_warp_axis(int base, int n, float d, int &i0, int &i1, float &a)
+{
+    const float dc = fminf(fmaxf(d, -(float)base), (float)(n - 1 - base));
+    const float f = floorf(dc);
+    a = dc - f;
+    i0 = base + (int)f;
+    i1 = min(i0 + 1, n - 1);
+}
+
 __device__ __forceinline__ float rfa_warp_voxel(int i, int j, int k, int nx, int ny, int nz, const float *__restrict__ theta,
                                                 float dx, float dy, float dz, float t_blood)
 {
-    const float d[3] = {dx, dy, dz};
-    const int base[3] = {i, j, k}, n[3] = {nx, ny, nz};
     int i0[3], i1[3];
     float a[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const float f = floorf(d[c]);
-        float frac = d[c] - f;
-        // clamp the shift first: |f| beyond the grid size saturates (and keeps the int conversion defined)
-        int p = base[c] + (int)fminf(fmaxf(f, -(float)n[c]), (float)n[c]);
-        if (p < 0) { p = 0; frac = 0.f; }
-        if (p >= n[c] - 1) { p = n[c] - 1; frac = 0.f; }
-        i0[c] = p;
-        i1[c] = min(p + 1, n[c] - 1);
-        a[c] = frac;
-    }
+    rfa_warp_axis(i, nx, dx, i0[0], i1[0], a[0]);
+    rfa_warp_axis(j, ny, dy, i0[1], i1[1], a[1]);
+    rfa_warp_axis(k, nz, dz, i0[2], i1[2], a[2]);
     const size_t sy = nx, sz = (size_t)nx * ny;
     const float *z0 = theta + (size_t)i0[2] * sz, *z1 = theta + (size_t)i1[2] * sz;
     const size_t r0 = (size_t)i0[1] * sy, r1 = (size_t)i1[1] * sy;
@@ -173,18 +174,18 @@ __global__ void rfa_warp_kernel(int nx, int ny, int nz, const float *__restrict_
     if (i >= nx || j >= ny) return;
     const size_t nvox = (size_t)nx * ny * nz;
     const size_t v = (size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * k);
+    const float sx = scale * ihx, sy_ = scale * ihy, sz_ = scale * ihz;       // mm -> voxels, scaled
     if constexpr (VEC == 4) {
         const float4 ux = *reinterpret_cast<const float4 *>(disp + v), uy = *reinterpret_cast<const float4 *>(disp + nvox + v),
                      uz = *reinterpret_cast<const float4 *>(disp + 2 * nvox + v);
         float4 o;
-        o.x = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, scale * ux.x * ihx, scale * uy.x * ihy, scale * uz.x * ihz, t_blood);
-        o.y = rfa_warp_voxel(i + 1, j, k, nx, ny, nz, theta, scale * ux.y * ihx, scale * uy.y * ihy, scale * uz.y * ihz, t_blood);
-        o.z = rfa_warp_voxel(i + 2, j, k, nx, ny, nz, theta, scale * ux.z * ihx, scale * uy.z * ihy, scale * uz.z * ihz, t_blood);
-        o.w = rfa_warp_voxel(i + 3, j, k, nx, ny, nz, theta, scale * ux.w * ihx, scale * uy.w * ihy, scale * uz.w * ihz, t_blood);
+        o.x = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, ux.x * sx, uy.x * sy_, uz.x * sz_, t_blood);
+        o.y = rfa_warp_voxel(i + 1, j, k, nx, ny, nz, theta, ux.y * sx, uy.y * sy_, uz.y * sz_, t_blood);
+        o.z = rfa_warp_voxel(i + 2, j, k, nx, ny, nz, theta, ux.z * sx, uy.z * sy_, uz.z * sz_, t_blood);
+        o.w = rfa_warp_voxel(i + 3, j, k, nx, ny, nz, theta, ux.w * sx, uy.w * sy_, uz.w * sz_, t_blood);
         *reinterpret_cast<float4 *>(out + v) = o;
     } else {
-        out[v] = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, scale * disp[v] * ihx, scale * disp[nvox + v] * ihy,
-                                scale * disp[2 * nvox + v] * ihz, t_blood);
+        out[v] = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, disp[v] * sx, disp[nvox + v] * sy_, disp[2 * nvox + v] * sz_, t_blood);
     }
 }
 
