@@ -39,11 +39,25 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "GVoxel-updates/s"
-STATE_BYTES_PER_VOXEL_PASS = 11.0    # 4 B theta read + 4 B theta write + 1 B state read + 2 B residual write
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the one
-# `ncu --set full` capture committed under profiles/ (r1_blocked_s3_ncu_full.md); keyed by (config, fused steps)
-NCU_TRAFFIC_BYTES = {("C4", 3): 729.5e6}
+# Algorithmic bytes per voxel per launch of the stepping kernel.  SURVEY.md 8(d) counts
+# 4 B theta read + 4 B theta write + 1 B label/flag byte + 1 B necrosis byte = 10 B, i.e. (8+2)/S per voxel-update with
+# S fused steps; that is the figure roofline.frac is taken on.  This build keeps the necrosis bit inside the state
+# byte (no second byte) but writes a 2-B fp16 residual image for the compensated accumulation: 4 + 4 + 1 + 2 = 11 B
+# is what the kernel itself must move, reported beside it as frac_11B.
+BYTES_SURVEY = {"theta_read": 4.0, "theta_write": 4.0, "label_byte": 1.0, "necrosis_byte": 1.0}
+BYTES_BUILD = {"theta_read": 4.0, "theta_write": 4.0, "state_byte_read": 1.0, "residual_fp16_write": 2.0}
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel, from the `ncu --set full`
+# captures summarised under profiles/.  Keyed by the variant string of the run (workload / fused steps / tile /
+# held-copy / conduction): a run whose variant has no capture prints "traffic": null.
+NCU_TRAFFIC = {
+    # variant: (bytes per launch, profile file)
+}
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def variant_key(workload, variant):
+    return "%s/S%d/%dx%d/hc%d/%s" % (workload, variant["fused_steps"], variant["tile_bx"], variant["tile_by"],
+                                     variant["held_copy"], "face" if variant["conduction"] else "eq12")
 
 
 def measured_peak():
@@ -248,50 +262,78 @@ def run_ours(args):
     stream = torch.cuda.Stream(device=dev)
 
     # ---- device-resident leg ------------------------------------------------------------------
+    hc_env = os.environ.get("RFA_HELD_COPY")          # A/B switch of the bench only; the library reads no environment
     with torch.cuda.stream(stream):
         sim = binding.from_workload(w, device=dev, stream=stream)
         sim.configure(args.kernel, args.fused)
+        if hc_env in ("0", "1"):
+            sim.configure_held_copy(int(hc_env))
         if args.conduction == "face":
             sim.set_conduction(binding.COND_FACE)
         sim.step(Wu)
         sim.synchronize()
         q0 = sim.query()
-        e0 = torch.cuda.Event(enable_timing=True)
-        e1 = torch.cuda.Event(enable_timing=True)
+        S = max(q0["fused_steps"], 1)
+        k_main, k_rem = K - K % S, K % S                # full S-step launches, then the remainder launch
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize(dev)
         with ClockSampler(local) as clk:
             e0.record(stream)
-            sim.step(K)
+            sim.step(k_main)
             e1.record(stream)
-            e1.synchronize()
-        torch.cuda.synchronize(dev)
-        if dist is not None:
-            dist.barrier()
-        ms_local = float(e0.elapsed_time(e1))
-        q1 = sim.query()
+            sim.step(k_rem)
+            e2.record(stream)
+            e2.synchronize()
+            torch.cuda.synchronize(dev)
+            if dist is not None:
+                dist.barrier()
+            ms_local = float(e0.elapsed_time(e2))
+            ms_main = float(e0.elapsed_time(e1))
+            q1 = sim.query()
+            # the timed region of a short run (the driver's --steps 20 is 2 ms) is shorter than one NVML sample: keep
+            # the same stepping loop running, untimed, until the sampler has seen >= 0.4 s under this load
+            t_probe = time.perf_counter()
+            while time.perf_counter() - t_probe < max(0.0, 0.4 - ms_local * 1e-3):
+                sim.step(30 * S)
+                sim.synchronize()
         variant = sim.query_variant()
         necro_all, necro_tissue = sim.necrotic_voxels(0)
         tmax = float(sim.get_temperature(0).max())
         sim.close()
         del sim
     launches = q1["kernel_launches"] - q0["kernel_launches"]
+    n_main = k_main // S
     ms, units = aggregate(ms_local, float(nvox_all) * K, dist, dev)
     gvox = units / (ms * 1e-3) / 1e9
     peak, peak_src = measured_peak()
 
-    # dominant kernel = the stepping kernel: the timed region holds nothing else on this stream
-    launch_us = ms_local * 1e3 / max(launches, 1)
-    bytes_per_launch = STATE_BYTES_PER_VOXEL_PASS * nvox_all
-    achieved = bytes_per_launch / (launch_us * 1e-6) / 1e9
+    # dominant kernel = the stepping kernel: the timed region holds nothing else on this stream.  Its launch time is
+    # taken over the full S-step launches only; the remainder launch (K % S steps) is reported separately.
+    blocked = q1["kernel"] == binding.KERNEL_BLOCKED
+    launch_us = ms_main * 1e3 / max(n_main, 1) if n_main else ms_local * 1e3 / max(launches, 1)
+    b_survey = sum(BYTES_SURVEY.values()) * nvox_all
+    b_build = sum(BYTES_BUILD.values()) * nvox_all
+    achieved = b_survey / (launch_us * 1e-6) / 1e9
+    vkey = variant_key(w.name, variant) if blocked else f"{w.name}/plain"
+    traffic, traffic_src = NCU_TRAFFIC.get(vkey, (None, None))
     roofline = {
-        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": NCU_TRAFFIC_BYTES.get((args.config, q1["fused_steps"])), "peak_source": peak_src,
-        "kernel": f"rfa_blocked_kernel<S={q1['fused_steps']}>" if q1["kernel"] == binding.KERNEL_BLOCKED else "rfa_plain_kernel",
-        "launches": launches, "avg_launch_us": launch_us, "algorithmic_bytes_per_launch": bytes_per_launch,
-        "fused_steps_per_launch": q1["fused_steps"],
-        # north_star's roofline-equivalent: one 4-B read + one 4-B write of the field per *time step*
+        # S = 1: one pass over the field per step, the HBM stream binds.  S >= 2: the kernel moves the same bytes per
+        # launch but does S steps of arithmetic on them; ncu shows the issue slots, not DRAM, as the busiest unit
+        # (profiles/): frac stays the true share of the HBM peak, it is just not what limits the kernel
+        "bound": "hbm" if (not blocked or S == 1) else "issue",
+        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": traffic, "traffic_source": traffic_src, "variant": vkey, "peak_source": peak_src,
+        "kernel": f"rfa_blocked_kernel<S={S}>" if blocked else "rfa_plain_kernel",
+        "launches": launches, "full_launches": n_main, "avg_launch_us": launch_us,
+        "remainder_launch": {"steps": k_rem, "us": (ms_local - ms_main) * 1e3} if k_rem else None,
+        "algorithmic_bytes_per_launch": b_survey, "bytes_per_voxel": BYTES_SURVEY,
+        "bytes_per_voxel_update": sum(BYTES_SURVEY.values()) / S,
+        "frac_11B": b_build / (launch_us * 1e-6) / 1e9 / peak, "bytes_per_voxel_build": BYTES_BUILD,
+        "fused_steps_per_launch": S,
+        # north_star's roofline-EQUIVALENT: voxel-updates/s x 8 B (one 4-B read + one 4-B write of the field per TIME
+        # STEP) over the copy peak.  A speed-up-equivalent that temporal blocking raises by design, not an HBM utilisation.
         "equiv_8B_frac": gvox / world * 8.0 / peak,
     }
 
@@ -310,6 +352,8 @@ def run_ours(args):
             s2 = binding.RfaSim(w.dims, w.spacing_mm, lab_h, w.table, w.t_blood, w.dt, batch=w.batch,
                                 device=dev, stream=stream)
             s2.configure(args.kernel, args.fused)
+            if hc_env in ("0", "1"):
+                s2.configure_held_copy(int(hc_env))
             if args.conduction == "face":
                 s2.set_conduction(binding.COND_FACE)
             for b, nd in enumerate(w.needles):
@@ -347,10 +391,10 @@ def run_ours(args):
                              "working set fits L2 (reported, not held to the HBM bar)",
                        "kernel": roofline["kernel"], "conduction": args.conduction, "variant": variant},
             "sim_steps_per_s": K / (ms * 1e-3) * (1 if world == 1 else world),
-            # BASELINE.json's "% of B200 HBM roofline": voxel-updates/s x 8 B (one read + one write of the fp32 field per
-            # time step, north_star) over the measured copy bandwidth; roofline.frac below uses the bytes the kernel
-            # must really move (11 B per voxel per launch of S fused steps), which temporal blocking shrinks on purpose
-            "hbm_roofline_equiv_frac": roofline["equiv_8B_frac"],
+            # BASELINE.json's "% of B200 HBM roofline" as north_star defines it: voxel-updates/s x 8 B (one read + one
+            # write of the fp32 field per time step) over the measured copy bandwidth -- a roofline-EQUIVALENT (speed-up
+            # over a one-step kernel at the copy peak), not an HBM utilisation; the true HBM fraction is roofline.frac
+            "roofline_equiv_8B_frac": roofline["equiv_8B_frac"],
             "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": launches,
             "clocks": clk.summary(),
             "check": {"t_max_c": tmax, "necrotic_voxels": necro_all, "necrotic_tissue_voxels": necro_tissue},
@@ -401,6 +445,95 @@ def run_warp(args):
     return 0
 
 
+def run_record(args):
+    """Row f2 and the paper's own regime (Alg. 2: ONE time iteration of Alg. 1 per displayed frame,
+    :330; probe curves of Fig. 6 / Fig. 14, :147).  Two legs on the configured volume, both one step per frame:
+      record   rfa_step_record(K, every=1): K single-step launches, each followed by the probe read-out kernel
+      handoff  the Alg. 2 frame loop: rfa_step(1) -> event -> a consumer on a SECOND stream reads the finished image
+               (rfa_current_frame; here a device-to-device copy into a "display" buffer stands in for the renderer)
+               while the next step runs into the other buffer; the step after that waits for the consumer's event,
+               because it overwrites the image the consumer was given."""
+    import torch
+    from cuda.bindings import runtime as cudart
+    from paper_1907_05709_b200 import binding, workloads as W
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    w = W.BENCH_CONFIGS[args.config]()
+    nx, ny, nz = w.dims
+    K = min(args.steps, 3000)
+    stream, side = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+    mz, my, mx = np.nonzero(w.needles[0].mask)
+    centre = (int(round(mx.mean())), int(round(my.mean())), int(round(mz.mean())))
+    probes = W.fig6_probes(w.dims, w.spacing_mm, centre).ravel()
+    with torch.cuda.stream(stream):
+        sim = binding.from_workload(w, device=dev, stream=stream)
+        sim.configure(args.kernel, 1)                      # one time step per launch: the interactive regime
+        hc_env = os.environ.get("RFA_HELD_COPY")
+        if hc_env in ("0", "1"):
+            sim.configure_held_copy(int(hc_env))
+        sim.set_probes(probes)
+        rec = torch.empty((K, probes.size), dtype=torch.float32, device=dev)
+        sim.step_record(max(args.warmup, 3), 1, out=rec)
+        q0 = sim.query()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with ClockSampler(dev.index or 0) as clk:
+            e0.record(stream)
+            sim.step_record(K, 1, out=rec)
+            e1.record(stream)
+            e1.synchronize()
+            ms_rec = float(e0.elapsed_time(e1))
+            q1 = sim.query()
+            # ---- Alg. 2 hand-off loop with an overlapped consumer
+            display = torch.empty(nx * ny * nz, dtype=torch.float32, device=dev)
+            prod = [torch.cuda.Event() for _ in range(K)]
+            cons = [torch.cuda.Event() for _ in range(K)]
+            nbytes = nx * ny * nz * 4
+            sim.step(3)
+            torch.cuda.synchronize(dev)
+            e0.record(stream)
+            for f in range(K):
+                if f >= 2:
+                    stream.wait_event(cons[f - 2])         # step f overwrites the image consumer f-2 was reading
+                sim.step(1)
+                prod[f].record(stream)
+                ptr, _ = sim.current_frame(0)
+                side.wait_event(prod[f])
+                (rc,) = cudart.cudaMemcpyAsync(display.data_ptr(), ptr, nbytes,
+                                               cudart.cudaMemcpyKind.cudaMemcpyDeviceToDevice, side.cuda_stream)
+                assert int(rc) == 0
+                cons[f].record(side)
+            e1.record(stream)
+            side.synchronize()
+            e1.synchronize()
+            torch.cuda.synchronize(dev)
+            ms_hand = float(e0.elapsed_time(e1))
+        variant = sim.query_variant()
+        last = rec[-1].cpu().numpy()
+        sim.close()
+    peak, peak_src = measured_peak()
+    fps_rec, fps_hand = K / (ms_rec * 1e-3), K / (ms_hand * 1e-3)
+    b_step = sum(BYTES_SURVEY.values()) * w.n_voxels
+    ach = b_step * fps_rec / 1e9
+    print(json.dumps({
+        "metric": "frames/s (Alg. 2 frame loop: one time step per frame, probes recorded every frame)",
+        "value": fps_rec, "unit": "frames/s", "n_gpus": 1, "steps": K, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_rec / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": w.name + " frame loop", "dims": list(w.dims), "probes": int(probes.size), "variant": variant,
+                   "paper_context": "PAPER.md:13/:290: > 480 Hz on a 256^2 x 234 volume (GTX 1080 / 1080 Ti), other hardware"},
+        "gvoxel_updates_per_s": w.n_voxels * fps_rec / 1e9,
+        "handoff": {"frames_per_s": fps_hand, "ms_per_frame": ms_hand / K, "gvoxel_updates_per_s": w.n_voxels * fps_hand / 1e9,
+                    "consumer": "device-to-device copy of the finished image (%d MiB) on a second stream, overlapped with "
+                                "the next step" % (nbytes >> 20)},
+        "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                     "peak_source": peak_src, "kernel": "rfa_blocked_kernel<S=1> + rfa_probe_kernel",
+                     "algorithmic_bytes_per_launch": b_step, "bytes_per_voxel": BYTES_SURVEY,
+                     "equiv_8B_frac": w.n_voxels * fps_rec * 8.0 / 1e9 / peak},
+        "gpu_launches": q1["kernel_launches"] - q0["kernel_launches"], "clocks": clk.summary(),
+        "check": {"probe_t_c_last_frame": [float(x) for x in last]}}), flush=True)
+    return 0
+
+
 def run_render(args):
     """Row f4 (headless view of the heat zone) on the C4 volume: K frames of 512 x 512 pixels, oblique view,
     0.5 mm steps.  Reported as frame time and trilinear samples per second (no roofline: the kernel is a
@@ -447,7 +580,7 @@ def main(argv=None):
     ap.add_argument("--fused", type=int, default=0, help="fused time steps per launch, 0 = library default")
     ap.add_argument("--conduction", default="eq12", choices=["eq12", "face"],
                     help="eq12: Eq. 12 as printed (default, the headline); face: conservative div(K grad T), row f1")
-    ap.add_argument("--op", default="step", choices=["step", "warp", "render"],
+    ap.add_argument("--op", default="step", choices=["step", "warp", "render", "record"],
                     help="step: the time-stepping hot path (the headline); warp: the Eq. 14 motion warp (row f3)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -460,6 +593,8 @@ def main(argv=None):
         return run_warp(args)
     if args.op == "render":
         return run_render(args)
+    if args.op == "record":
+        return run_record(args)
     return run_ours(args)
 
 

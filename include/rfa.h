@@ -19,8 +19,10 @@
  * DESIGN.md section 5); per-label coefficients are derived in fp64 on the host and rounded once.
  *
  * Memory: "host" pointers are ordinary host memory.  Pointers documented "host or device" may be
- * either (the library asks the CUDA runtime).  The library copies what it is given during the call;
- * the caller keeps ownership of all its buffers.  Device state lives in the caller's workspace
+ * either (the library asks the CUDA runtime).  Host inputs are copied during the call; device inputs are
+ * read asynchronously on the simulation's stream (stated per call); the caller keeps ownership of all its
+ * buffers.  A simulation lives on the CUDA device that is current at rfa_create: every later call switches
+ * to that device for its own work and restores the caller's current device before it returns.  Device state lives in the caller's workspace
  * (see rfa_workspace_bytes) or, if none is given, in memory the library allocates and frees.
  *
  * Errors: every int-returning call returns RFA_OK (0) or a negative code; no exception crosses the
@@ -106,8 +108,11 @@ int rfa_create(rfa_sim **out, const int dims[3], const float spacing_mm[3], cons
                void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /* Place (or move, or with RFA_SRC_OFF remove) the needle of one scenario.
- *   tip_mm, axis  metadata only, validated for finiteness (the mask is authoritative); may be NULL
- *   mask          host or device, nx*ny*nz bytes, nonzero = electrode voxel; ignored for RFA_SRC_OFF
+ *   tip_mm, axis  metadata (the mask is authoritative), validated when given: tip_mm must lie inside the grid
+ *                 [0, n*spacing] mm per axis and |axis| must be 1 +- 1e-3, else RFA_E_INVALID; either may be NULL
+ *   mask          host or device, nx*ny*nz bytes, nonzero = electrode voxel; ignored for RFA_SRC_OFF.
+ *                 A host mask is copied before the call returns.  A DEVICE mask is read asynchronously on the
+ *                 simulation's stream: keep it valid and unchanged until rfa_synchronize (or a stream event).
  *   DIRICHLET: mask voxels are set to `value` deg C and held, overriding the label (R-15)
  *   POWER:     mask voxels get +value W/m^3 in the bracket of Eq. 12; a held label stays held (R-17)
  * Voxels of a previous needle are released: they keep their temperature and follow their label (R-16). */
@@ -115,7 +120,9 @@ int rfa_set_needle(rfa_sim *s, int scenario, const float tip_mm[3], const float 
                    const uint8_t *mask, int mode, float value);
 
 /* Overwrite the temperature image of one scenario (deg C, host or device, nx*ny*nz floats);
- * necrosis |= (T >= 60).  Held voxels keep whatever is written here. */
+ * necrosis |= (T >= 60).  Held voxels keep whatever is written here.  A host image is copied before the call
+ * returns; a DEVICE image is read asynchronously on the simulation's stream (keep it valid until rfa_synchronize
+ * or a stream event). */
 int rfa_set_temperature(rfa_sim *s, int scenario, const float *t_c);
 
 /* Advance every scenario by n time steps (n >= 0).  Asynchronous. */
@@ -145,8 +152,13 @@ int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launche
  * out = { fused_steps, tile_bx, tile_by, ctas_launched, held_copy, conduction }.  held_copy = 1: the kernel variant in
  * which warps whose voxels are all held copy their rows instead of evaluating the bracket (Alg. 1's else-branch,
  * PAPER.md:313; bit-identical), chosen at rfa_create when at least 1/8 of the volume carries a held label
- * (environment variable RFA_HELD_COPY=0/1 overrides, for A/B measurements).  Zeros for the plain kernel. */
+ * (rfa_configure_held_copy overrides, for A/B measurements).  Zeros for the plain kernel. */
 int rfa_query_variant(rfa_sim *s, int out[6]);
+
+/* Force the held-copy kernel variant on or off, or hand the choice back to the library (what rfa_create decided
+ * from the share of held labels).  All settings give bit-identical fields; the library reads no environment variable. */
+enum { RFA_HELD_COPY_AUTO = -1, RFA_HELD_COPY_OFF = 0, RFA_HELD_COPY_ON = 1 };
+int rfa_configure_held_copy(rfa_sim *s, int mode);
 
 /* Host-only view of the blocked kernel's launch plan for a grid (no GPU needed; used by the unit tests
  * and the bench report).  resident_ctas = CTAs that can be co-resident (SM count x occupancy).
@@ -198,7 +210,8 @@ int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp, float scal
  *   A sample counts if it lies inside the box of voxel centres; there T is interpolated trilinearly.
  *   tmax[py*W+px]  = maximum of T over the ray's samples (t_blood if none lies inside)            [deg C]
  *   depth[py*W+px] = m*step_mm of the first sample with T >= iso_c, or -1 if there is none        [mm]
- * Outputs: host or device, W*H floats each; depth may be NULL.  Reads the state only.  Synchronous. */
+ * Outputs: host or device, W*H floats each (1 <= W*H <= 2^28); depth may be NULL.  Host images are staged in a
+ * library-owned device buffer that grows on demand.  Reads the state only.  Synchronous. */
 typedef struct rfa_view {
     float dir[3];      /* viewing direction (any non-zero length) */
     float up[3];       /* not parallel to dir */

@@ -21,12 +21,13 @@ KERNEL_AUTO, KERNEL_PLAIN, KERNEL_BLOCKED = 0, 1, 2
 TISSUE_HELD = 1
 MAX_TISSUES = 16
 COND_EQ12, COND_FACE = 0, 1
+HELD_COPY_AUTO, HELD_COPY_OFF, HELD_COPY_ON = -1, 0, 1
 
 # every symbol include/rfa.h declares
 EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
-    "rfa_set_conduction", "rfa_query", "rfa_query_variant", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
+    "rfa_set_conduction", "rfa_query", "rfa_query_variant", "rfa_configure_held_copy", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
     "rfa_warp_temperature", "rfa_render_zone",
     "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
@@ -93,6 +94,8 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_query.restype = ctypes.c_int
     lib.rfa_query_variant.argtypes = [vp, ctypes.POINTER(ctypes.c_int)]
     lib.rfa_query_variant.restype = ctypes.c_int
+    lib.rfa_configure_held_copy.argtypes = [vp, ctypes.c_int]
+    lib.rfa_configure_held_copy.restype = ctypes.c_int
     lib.rfa_plan_query.argtypes = [i3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
     lib.rfa_plan_query.restype = ctypes.c_int
     lib.rfa_set_probes.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int64)]
@@ -236,6 +239,9 @@ class RfaSim:
 
     def configure(self, kernel: int = KERNEL_AUTO, fused_steps: int = 0):
         _check(self._lib.rfa_configure(self._handle, int(kernel), int(fused_steps)))
+
+    def configure_held_copy(self, mode: int = HELD_COPY_AUTO):
+        _check(self._lib.rfa_configure_held_copy(self._handle, int(mode)))
 
     def set_conduction(self, mode: int):
         _check(self._lib.rfa_set_conduction(self._handle, int(mode)))

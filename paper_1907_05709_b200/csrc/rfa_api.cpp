@@ -65,7 +65,44 @@ struct rfa_sim {
     int n_probes = 0;
     float *record = nullptr;             // device staging of rfa_step_record (library-owned, grows on demand)
     size_t record_cap = 0;               // floats
+    float *stage = nullptr;              // device staging of host displacement fields / host images (library-owned,
+    size_t stage_cap = 0;                // grows on demand; floats)
+    int device = 0;                      // the CUDA device the simulation lives on (current device at rfa_create)
+    int held_copy_auto = 0;              // what rfa_create chose for the held-copy variant (RFA_HELD_COPY_AUTO)
 };
+
+// Every entry point that touches the device runs on the simulation's own device, whatever the caller's current
+// device is, and puts the caller's device back on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const rfa_sim *s)
+    {
+        if (s && cudaGetDevice(&prev) == cudaSuccess && prev != s->device) switched = cudaSetDevice(s->device) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
+// library-owned device staging buffer of at least `floats` floats (the stream is drained before it is replaced)
+static int ensure_stage(rfa_sim *s, size_t floats)
+{
+    if (s->stage_cap >= floats) return RFA_OK;
+    cudaError_t e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return RFA_E_CUDA;
+    if (s->stage) cudaFree(s->stage);
+    s->stage = nullptr;
+    s->stage_cap = 0;
+    e = cudaMalloc((void **)&s->stage, floats * sizeof(float));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return RFA_E_NOMEM;
+    }
+    s->stage_cap = floats;
+    return RFA_OK;
+}
 
 // ------------------------------------------------------------------------------------------------
 // workspace layout
@@ -315,10 +352,21 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     for (int l = 0; l < n_tissue; ++l)
         if (!tissue_ok(table[l])) return fail(RFA_E_INVALID, "tissue row %d: non-finite or non-positive constants", l);
     const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
+    // one pass over the host label volume: histogram of the label ids (range check, held volume)
+    size_t hist[256] = {0};
     {
-        unsigned mx = 0;
-        for (size_t v = 0; v < nvox; ++v) mx = std::max<unsigned>(mx, labels[v]);
-        if ((int)mx >= n_tissue) return fail(RFA_E_INVALID, "label id %u >= n_tissue %d", mx, n_tissue);
+        size_t h4[4][256] = {{0}};                           // four independent counters: no store-to-load chain
+        size_t v = 0;
+        for (; v + 4 <= nvox; v += 4) {
+            h4[0][labels[v]]++;
+            h4[1][labels[v + 1]]++;
+            h4[2][labels[v + 2]]++;
+            h4[3][labels[v + 3]]++;
+        }
+        for (; v < nvox; ++v) h4[0][labels[v]]++;
+        for (int l = 0; l < 256; ++l) hist[l] = h4[0][l] + h4[1][l] + h4[2][l] + h4[3][l];
+        for (int l = 255; l >= n_tissue; --l)
+            if (hist[l]) return fail(RFA_E_INVALID, "label id %d >= n_tissue %d", l, n_tissue);
     }
     const double stab = rfa_stability_number(spacing_mm, table, n_tissue, dt_s);
     if (stab < 0) return fail(RFA_E_INVALID, "invalid constants");
@@ -362,12 +410,12 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     {
         // Held-copy kernel variant (warps whose voxels are all held copy their rows instead of evaluating the
         // bracket; bit-identical): worth its extra vote per level only where a good part of the volume is held
-        // (the air around the body in C4: +11 %; -7 % on the 128^3 phantoms without it).  RFA_HELD_COPY=0/1 overrides.
+        // (the air around the body in C4: +11 %; -7 % on the 128^3 phantoms without it).  rfa_configure_held_copy overrides.
         size_t n_held = 0;
-        for (size_t v = 0; v < nvox; ++v) n_held += (table[labels[v]].flags & RFA_TISSUE_HELD) ? 1 : 0;
-        s->g.held_copy = n_held * 8 >= nvox ? 1 : 0;
-        const char *hc = std::getenv("RFA_HELD_COPY");
-        if (hc && (hc[0] == '0' || hc[0] == '1')) s->g.held_copy = hc[0] - '0';
+        for (int l = 0; l < n_tissue; ++l)
+            if (table[l].flags & RFA_TISSUE_HELD) n_held += hist[l];
+        s->held_copy_auto = n_held * 8 >= nvox ? 1 : 0;
+        s->g.held_copy = s->held_copy_auto;
     }
     s->g.thr = (float)(60.0 - (double)t_blood_c);            // T >= 60 C  (R-11)
     s->table.assign(table, table + n_tissue);
@@ -383,10 +431,22 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
         cudaGetLastError();
         return fail(RFA_E_CUDA, "no CUDA device (%s); librfa has no CPU fallback", e != cudaSuccess ? cudaGetErrorString(e) : "count = 0");
     }
+    if (cudaGetDevice(&s->device) != cudaSuccess) {
+        delete s;
+        cudaGetLastError();
+        return fail(RFA_E_CUDA, "cudaGetDevice failed");
+    }
     if (workspace) {
-        if (!is_device_ptr(workspace)) {
+        cudaPointerAttributes at{};
+        if (cudaPointerGetAttributes(&at, workspace) != cudaSuccess ||
+            (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)) {
             delete s;
+            cudaGetLastError();
             return fail(RFA_E_INVALID, "workspace is not device memory");
+        }
+        if (at.type == cudaMemoryTypeDevice && at.device != s->device) {
+            delete s;
+            return fail(RFA_E_INVALID, "workspace lives on device %d, the current device is %d", at.device, s->device);
         }
         s->ws = (unsigned char *)workspace;
     } else {
@@ -450,10 +510,14 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
 extern "C" void rfa_destroy(rfa_sim *s)
 {
     if (!s) return;
-    cudaStreamSynchronize(s->stream);
-    if (s->own_ws) cudaFree(s->ws);
-    if (s->probes) cudaFree(s->probes);
-    if (s->record) cudaFree(s->record);
+    {
+        DeviceGuard dg(s);
+        cudaStreamSynchronize(s->stream);
+        if (s->own_ws) cudaFree(s->ws);
+        if (s->probes) cudaFree(s->probes);
+        if (s->record) cudaFree(s->record);
+        if (s->stage) cudaFree(s->stage);
+    }
     delete s;
 }
 
@@ -462,12 +526,27 @@ extern "C" int rfa_set_needle(rfa_sim *s, int scenario, const float tip_mm[3], c
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     if (mode != RFA_SRC_OFF && mode != RFA_SRC_DIRICHLET && mode != RFA_SRC_POWER) return fail(RFA_E_INVALID, "bad source mode %d", mode);
     if (mode != RFA_SRC_OFF && !mask) return fail(RFA_E_INVALID, "mask is null");
     if (mode != RFA_SRC_OFF && !std::isfinite(value)) return fail(RFA_E_INVALID, "source value must be finite");
-    for (int a = 0; a < 3; ++a) {
-        if (tip_mm && !std::isfinite(tip_mm[a])) return fail(RFA_E_INVALID, "tip position must be finite");
-        if (axis && !std::isfinite(axis[a])) return fail(RFA_E_INVALID, "axis must be finite");
+    // tip / axis are metadata (the mask is authoritative), but a tip outside the grid or a non-unit axis means the
+    // caller's geometry and its mask disagree: reject
+    if (tip_mm) {
+        const int n[3] = {s->g.nx, s->g.ny, s->g.nz};
+        for (int a = 0; a < 3; ++a) {
+            const double ext = n[a] * s->h_m[a] * 1.0e3;
+            if (!std::isfinite(tip_mm[a]) || tip_mm[a] < -1.0e-3 || tip_mm[a] > ext + 1.0e-3)
+                return fail(RFA_E_INVALID, "tip position %g mm outside the grid [0, %g] mm along axis %d", (double)tip_mm[a], ext, a);
+        }
+    }
+    if (axis) {
+        double n2 = 0;
+        for (int a = 0; a < 3; ++a) {
+            if (!std::isfinite(axis[a])) return fail(RFA_E_INVALID, "axis must be finite");
+            n2 += (double)axis[a] * axis[a];
+        }
+        if (std::fabs(std::sqrt(n2) - 1.0) > 1.0e-3) return fail(RFA_E_INVALID, "axis must be a unit vector (|axis| = %.6f)", std::sqrt(n2));
     }
     const uint8_t *mdev = nullptr;
     cudaError_t e;
@@ -498,6 +577,7 @@ extern "C" int rfa_set_temperature(rfa_sim *s, int scenario, const float *t_c)
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     if (!t_c) return fail(RFA_E_INVALID, "t_c is null");
     const float *src = t_c;
     cudaError_t e;
@@ -527,6 +607,15 @@ extern "C" int rfa_configure(rfa_sim *s, int kernel, int fused_steps)
         return fail(RFA_E_INVALID, "the blocked kernel needs nx %% 4 == 0 and ny, nz >= fused steps (grid %dx%dx%d, fused %d)", s->g.nx, s->g.ny, s->g.nz, f);
     s->kernel = kernel;
     s->fused = f;
+    return RFA_OK;
+}
+
+extern "C" int rfa_configure_held_copy(rfa_sim *s, int mode)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (mode != RFA_HELD_COPY_AUTO && mode != RFA_HELD_COPY_OFF && mode != RFA_HELD_COPY_ON)
+        return fail(RFA_E_INVALID, "bad held-copy mode %d", mode);
+    s->g.held_copy = mode == RFA_HELD_COPY_AUTO ? s->held_copy_auto : (mode == RFA_HELD_COPY_ON ? 1 : 0);
     return RFA_OK;
 }
 
@@ -602,6 +691,7 @@ extern "C" int rfa_query_variant(rfa_sim *s, int out[6])
 extern "C" int rfa_step(rfa_sim *s, int n)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    DeviceGuard dg(s);
     if (n < 0) return fail(RFA_E_INVALID, "n must be >= 0");
     return advance(s, n);
 }
@@ -609,6 +699,7 @@ extern "C" int rfa_step(rfa_sim *s, int n)
 extern "C" int rfa_set_probes(rfa_sim *s, int n_probes, const int64_t *index)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    DeviceGuard dg(s);
     if (n_probes < 0 || (n_probes > 0 && !index)) return fail(RFA_E_INVALID, "bad probe list");
     const long long total = (long long)s->nvox * s->g.batch;
     for (int p = 0; p < n_probes; ++p)
@@ -631,6 +722,7 @@ extern "C" int rfa_set_probes(rfa_sim *s, int n_probes, const int64_t *index)
 extern "C" int rfa_step_record(rfa_sim *s, int n, int every, float *out)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    DeviceGuard dg(s);
     if (n < 0 || every < 1 || (n % every) != 0) return fail(RFA_E_INVALID, "n must be a non-negative multiple of every >= 1");
     if (s->n_probes == 0) return fail(RFA_E_INVALID, "no probes set (rfa_set_probes)");
     if (!out) return fail(RFA_E_INVALID, "out is null");
@@ -672,6 +764,7 @@ extern "C" int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_d
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     if (!theta_dev) return fail(RFA_E_INVALID, "theta_dev is null");
     *theta_dev = s->theta[s->cur] + (size_t)scenario * s->nvox;
     if (t_blood_c) *t_blood_c = (float)s->t_blood;
@@ -682,30 +775,35 @@ extern "C" int rfa_warp_temperature(rfa_sim *s, int scenario, const float *disp,
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     if (!disp || !out) return fail(RFA_E_INVALID, "null argument");
     if (!std::isfinite(scale)) return fail(RFA_E_INVALID, "scale must be finite");
     const size_t nvox = s->nvox;
     const float *ddev = disp;
-    float *tmp = nullptr;
     cudaError_t e;
-    if (!is_device_ptr(disp)) {
-        e = cudaMalloc((void **)&tmp, 3 * nvox * sizeof(float));
-        if (e != cudaSuccess) { cudaGetLastError(); return fail(RFA_E_NOMEM, "cudaMalloc of the displacement staging failed"); }
-        e = cudaMemcpyAsync(tmp, disp, 3 * nvox * sizeof(float), cudaMemcpyHostToDevice, s->stream);
-        if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(e, "displacement upload"); }
-        ddev = tmp;
+    const bool din = is_device_ptr(disp), dev = is_device_ptr(out);
+    if (!din) {
+        // host field: staged through the library-owned buffer (kept for the next call, freed by rfa_destroy)
+        rc = ensure_stage(s, 3 * nvox);
+        if (rc) return fail(rc, "staging buffer for the displacement field (%zu floats)", 3 * nvox);
+        e = cudaMemcpyAsync(s->stage, disp, 3 * nvox * sizeof(float), cudaMemcpyHostToDevice, s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "displacement upload");
+        ddev = s->stage;
     }
-    const bool dev = is_device_ptr(out);
     float *dst = dev ? out : (float *)s->scratch;
     const float inv_h[3] = {(float)(1.0e-3 / s->h_m[0]), (float)(1.0e-3 / s->h_m[1]), (float)(1.0e-3 / s->h_m[2])};
     e = rfa_launch_warp(s->g, scenario, s->theta[s->cur], ddev, scale, inv_h, dst, s->stream);
     s->launches++;
-    if (e == cudaSuccess && !dev) e = cudaMemcpyAsync(out, dst, nvox * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
-    // device field in, device image out: nothing of the caller's is touched after the launch -> asynchronous
-    cudaError_t e2 = (tmp != nullptr || !dev) ? cudaStreamSynchronize(s->stream) : cudaSuccess;
-    if (tmp) cudaFree(tmp);
     if (e != cudaSuccess) return cuda_fail(e, "warp kernel");
-    if (e2 != cudaSuccess) return cuda_fail(e2, "warp_temperature");
+    if (!dev) {
+        e = cudaMemcpyAsync(out, dst, nvox * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "warp download");
+    }
+    // device field in, device image out: nothing of the caller's host memory is touched -> asynchronous
+    if (!din || !dev) {
+        e = cudaStreamSynchronize(s->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "warp_temperature");
+    }
     return RFA_OK;
 }
 
@@ -713,9 +811,10 @@ extern "C" int rfa_render_zone(rfa_sim *s, int scenario, const rfa_view *view, f
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     if (!view || !tmax) return fail(RFA_E_INVALID, "null argument");
-    if (view->width < 1 || view->height < 1 || (long long)view->width * view->height > (long long)s->nvox / 2 + 4096)
-        return fail(RFA_E_INVALID, "image of %d x %d pixels: need 1 <= W*H <= nx*ny*nz/2", view->width, view->height);
+    if (view->width < 1 || view->height < 1 || (long long)view->width * view->height > (1LL << 28))
+        return fail(RFA_E_INVALID, "image of %d x %d pixels: need 1 <= W*H <= 2^28", view->width, view->height);
     if (!(view->pixel_mm > 0.f) || !(view->step_mm > 0.f) || !std::isfinite(view->pixel_mm) || !std::isfinite(view->step_mm) ||
         !std::isfinite(view->iso_c))
         return fail(RFA_E_INVALID, "pixel_mm and step_mm must be positive and finite, iso_c finite");
@@ -754,10 +853,15 @@ extern "C" int rfa_render_zone(rfa_sim *s, int scenario, const rfa_view *view, f
     if (ns > 1.0e6) return fail(RFA_E_INVALID, "step_mm too small: %.0f samples per ray", ns);
     ray.n_samples = (int)ns;
     const size_t npix = (size_t)view->width * view->height;
-    // host outputs are staged in the scratch volume (4 bytes per voxel): tmax in its first half, depth in the second
+    // host outputs are staged in the library-owned staging buffer (grows on demand): tmax first, depth behind it
     const bool tdev = is_device_ptr(tmax), ddev = depth ? is_device_ptr(depth) : true;
-    float *tdst = tdev ? tmax : (float *)s->scratch;
-    float *ddst = depth ? (ddev ? depth : (float *)s->scratch + s->nvox / 2) : nullptr;
+    const size_t n_staged = (tdev ? 0 : npix) + ((depth && !ddev) ? npix : 0);
+    if (n_staged) {
+        rc = ensure_stage(s, n_staged);
+        if (rc) return fail(rc, "staging buffer for the images (%zu floats)", n_staged);
+    }
+    float *tdst = tdev ? tmax : s->stage;
+    float *ddst = depth ? (ddev ? depth : s->stage + (tdev ? 0 : npix)) : nullptr;
     const float iso_theta = (float)((double)view->iso_c - s->t_blood);
     cudaError_t e = rfa_launch_render(s->g, scenario, ray, s->theta[s->cur], iso_theta, tdst, ddst, s->stream);
     s->launches++;
@@ -773,6 +877,7 @@ extern "C" int rfa_render_zone(rfa_sim *s, int scenario, const rfa_view *view, f
 extern "C" int rfa_synchronize(rfa_sim *s)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    DeviceGuard dg(s);
     cudaError_t e = cudaStreamSynchronize(s->stream);
     if (e != cudaSuccess) return cuda_fail(e, "synchronize");
     return RFA_OK;
@@ -782,6 +887,7 @@ extern "C" int rfa_get_temperature(rfa_sim *s, int scenario, float *out)
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     if (!out) return fail(RFA_E_INVALID, "out is null");
     const bool dev = is_device_ptr(out);
     float *dst = dev ? out : (float *)s->scratch;
@@ -801,6 +907,7 @@ extern "C" int rfa_get_necrosis(rfa_sim *s, int scenario, uint8_t *out)
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     if (!out) return fail(RFA_E_INVALID, "out is null");
     const bool dev = is_device_ptr(out);
     uint8_t *dst = dev ? out : s->scratch;
@@ -820,6 +927,7 @@ extern "C" int rfa_necrotic_voxels(rfa_sim *s, int scenario, int64_t *all_voxels
 {
     int rc = check_sim(s, scenario);
     if (rc) return rc;
+    DeviceGuard dg(s);
     cudaError_t e = rfa_launch_count(s->g, scenario, s->state, s->label_held_mask, s->counters, s->stream);
     s->launches++;
     if (e != cudaSuccess) return cuda_fail(e, "count kernel");

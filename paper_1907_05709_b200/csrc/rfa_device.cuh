@@ -63,9 +63,11 @@ __device__ __forceinline__ float rfa_face_correction(float t, float xm, float xp
                                                      float zp, float kxm, float kxp, float kym, float kyp,
                                                      float kzm, float kzp, float wx, float wy, float wz)
 {
-    const float cx = __fmaf_rn(kxm, __fsub_rn(xm, t), __fmul_rn(kxp, __fsub_rn(xp, t)));
-    const float cy = __fmaf_rn(kym, __fsub_rn(ym, t), __fmul_rn(kyp, __fsub_rn(yp, t)));
-    const float cz = __fmaf_rn(kzm, __fsub_rn(zm, t), __fmul_rn(kzp, __fsub_rn(zp, t)));
+    // both products are rounded before they are added: the result is bit-symmetric under swapping the two sides of
+    // an axis, like rfa_bracket, which is what lets the blocked kernel load mirrored y/z halos at the outer faces
+    const float cx = __fadd_rn(__fmul_rn(kxm, __fsub_rn(xm, t)), __fmul_rn(kxp, __fsub_rn(xp, t)));
+    const float cy = __fadd_rn(__fmul_rn(kym, __fsub_rn(ym, t)), __fmul_rn(kyp, __fsub_rn(yp, t)));
+    const float cz = __fadd_rn(__fmul_rn(kzm, __fsub_rn(zm, t)), __fmul_rn(kzp, __fsub_rn(zp, t)));
     return __fmaf_rn(wz, cz, __fmaf_rn(wy, cy, __fmul_rn(wx, cx)));
 }
 

@@ -13,7 +13,7 @@ struct RfaGrid {
     float thr;          // necrosis threshold in theta = T - T_a
     float t_blood;
     int held_copy;      // 1: kernel variant in which warps of held voxels only copy their rows (Alg. 1 :313);
-                        // chosen by rfa_create when >= 1/8 of the volume carries a held label (RFA_HELD_COPY=0/1 overrides)
+                        // chosen by rfa_create when >= 1/8 of the volume carries a held label (rfa_configure_held_copy overrides)
 };
 
 // Plan of the temporally blocked kernel for one launch geometry.

@@ -6,6 +6,7 @@
 //
 // Every stepping kernel evaluates rfa_bracket() + rfa_advance() (rfa_device.cuh) with the same operands
 // in the same order, so all variants produce bit-identical fields.
+#include <atomic>
 #include <cstdio>
 
 #include <cuda_fp16.h>
@@ -372,6 +373,7 @@ struct TbCfg {
     static constexpr size_t SMEM = RING_T + EXCH + RING_S + RSM + TAB + KAP;
 };
 
+#define RFA_MAX_DEVICES 64
 typedef unsigned long long u64;
 __device__ __forceinline__ u64 pk(float lo, float hi)
 {
@@ -956,11 +958,15 @@ static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_
 {
     using K = TbKernel<S, CONS, SHAPE, HC>;
     auto kern = K::get();
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::C::SMEM);
+    // the dynamic shared-memory opt-in is a per-DEVICE function attribute: remember it per device ordinal
+    static std::atomic<bool> attr_set[RFA_MAX_DEVICES];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= RFA_MAX_DEVICES || !attr_set[dev].load(std::memory_order_acquire)) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::C::SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        if (dev >= 0 && dev < RFA_MAX_DEVICES) attr_set[dev].store(true, std::memory_order_release);
     }
     kern<<<grid, K::C::NT, K::C::SMEM, st>>>(p);
     return cudaGetLastError();

@@ -469,16 +469,23 @@ def breathing_field(dims, amp_mm=(2.0, 4.0, 12.0)) -> np.ndarray:
     return out
 
 
+def with_smooth_field(w: Workload, amp_c: float = 8.0, periods=(64.0, 48.0, 32.0)) -> Workload:
+    """Gives workload w a smooth non-uniform initial temperature 37 + amp cos cos cos (deg C; periods in voxels
+    along x, y, z), so that every voxel of the volume changes from the first step on (held labels keep what is
+    written): the field-wide full-size parity cases, where a uniform 37 C far field would hide tile seams."""
+    nx, ny, nz = w.dims
+    cx = np.cos(2.0 * np.pi * (np.arange(nx) + 0.5) / periods[0])
+    cy = np.cos(2.0 * np.pi * (np.arange(ny) + 0.5) / periods[1])
+    cz = np.cos(2.0 * np.pi * (np.arange(nz) + 0.5) / periods[2])
+    w.t0 = 37.0 + amp_c * cz[:, None, None] * cy[None, :, None] * cx[None, None, :]
+    return w
+
+
 def c4_face_case(steps: int = 400) -> Workload:
     """C4 body model with a smooth non-uniform initial temperature (37 + 8 cos cos cos, deg C), so that heat
     crosses every tissue interface from the first step: the full-size case of the conservative conduction
     term (row f1).  Needle as in C4."""
-    w = c4_body(steps=steps)
-    nx, ny, nz = w.dims
-    cx = np.cos(2.0 * np.pi * (np.arange(nx) + 0.5) / 64.0)
-    cy = np.cos(2.0 * np.pi * (np.arange(ny) + 0.5) / 48.0)
-    cz = np.cos(2.0 * np.pi * (np.arange(nz) + 0.5) / 32.0)
-    w.t0 = 37.0 + 8.0 * cz[:, None, None] * cy[None, :, None] * cx[None, None, :]
+    w = with_smooth_field(c4_body(steps=steps))
     w.name = "C4F"
     return w
 

@@ -12,7 +12,13 @@ Per config <C> it writes tests/golden/<C>_golden.npz with, at checkpoints (steps
 and for the final state: a 32^3 crop around the needle centroid (crop_lo, crop_T), the bit-packed
 necrosis mask, necrotic voxel counts (all / without held-label and needle voxels), the voxels whose
 temperature lies within 2e-3 C of 60 C (band_idx, band_T: the exempt band of BASELINE.json's
-north_star is 1e-3), the field sum and maximum, a fingerprint of the inputs, and the oracle's speed.
+north_star is 1e-3), the field sum and maximum, a fingerprint of the inputs, and the oracle's speed,
+and the WHOLE final field in a compact form (field_*): with T_init = t_init[label] (the label ->
+temperature image of PAPER.md:139, which a test rebuilds from the inputs alone), the bounding box of the
+voxels with |T - T_init| > 1e-6 C is stored as integer codes rint((T - T_init) / field_q), field_q = 1e-5 C
+(so a stored value is within field_q / 2 of the oracle's), together with the largest |T - T_init| outside
+the box (field_outside_max <= 1e-6).  A test that finds its field within TOL - field_q / 2 of the decoded
+box and within TOL - field_outside_max of T_init elsewhere has shown |T - T_oracle| <= TOL at EVERY voxel.
 For the batched config C5 the same is stored per scenario (fewer samples each).  "C4F" = the C4 body model with a
 smooth non-uniform initial field and the conservative conduction term (row f1), 400 steps, with extra
 samples on tissue interfaces.
@@ -69,6 +75,29 @@ def interface_indices(w, n: int, seed: int) -> np.ndarray:
     return (x[pick] + nx * (y[pick] + ny * z[pick])).astype(np.int64)
 
 
+FIELD_Q = 1.0e-5        # deg C per code of the compact field
+FIELD_EPS = 1.0e-6      # voxels that moved less than this from T_init stay outside the stored box
+
+
+def compact_field(T, w) -> dict:
+    """The whole fp64 field as integer codes over the bounding box of the voxels that left T_init (see the
+    module docstring).  Data handling only: no method arithmetic."""
+    dev = T - np.asarray(w.table["t_init"], dtype=np.float64)[w.labels]
+    moved = np.abs(dev) > FIELD_EPS
+    if not moved.any():
+        lo, hi = np.zeros(3, np.int64), np.ones(3, np.int64)
+    else:
+        lo = np.array([np.nonzero(moved.any(axis=tuple(a for a in range(3) if a != ax)))[0][0] for ax in range(3)])
+        hi = np.array([np.nonzero(moved.any(axis=tuple(a for a in range(3) if a != ax)))[0][-1] + 1 for ax in range(3)])
+    box = dev[lo[0]:hi[0], lo[1]:hi[1], lo[2]:hi[2]]
+    codes = np.rint(box / FIELD_Q)
+    assert np.abs(codes).max() < 2 ** 31 and np.abs(codes * FIELD_Q - box).max() <= 0.5 * FIELD_Q * (1 + 1e-9)
+    out = np.abs(dev)
+    out[lo[0]:hi[0], lo[1]:hi[1], lo[2]:hi[2]] = 0.0
+    return {"field_q": np.float64(FIELD_Q), "field_lo": lo.astype(np.int64), "field_codes": codes.astype(np.int32),
+            "field_outside_max": np.float64(out.max())}
+
+
 def run_scenario(w, scenario: int, n_samples: int, crop: int, checkpoints, conservative: bool = False):
     nx, ny, nz = w.dims
     sim = rfa_oracle.OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt, conservative=conservative)
@@ -100,6 +129,7 @@ def run_scenario(w, scenario: int, n_samples: int, crop: int, checkpoints, conse
     crop_T = T[lo[0]:lo[0] + crop, lo[1]:lo[1] + crop, lo[2]:lo[2] + crop].copy()
     flat = T.ravel()
     band = np.nonzero(np.abs(flat - 60.0) <= 2e-3)[0]
+    field = compact_field(T, w)
     res = {
         "sample_idx": idx,
         "sample_T": np.stack(out_T),
@@ -117,6 +147,7 @@ def run_scenario(w, scenario: int, n_samples: int, crop: int, checkpoints, conse
         "oracle_gvox_per_s": np.float64(w.n_voxels * checkpoints[-1] / secs / 1e9),
         "oracle_threads": np.int64(rfa_oracle.num_threads()),
     }
+    res.update(field)
     return res
 
 
