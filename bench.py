@@ -312,20 +312,21 @@ def run_ours(args):
     # dominant kernel = the stepping kernel: the timed region holds nothing else on this stream.  Its launch time is
     # taken over the full S-step launches only; the remainder launch (K % S steps) is reported separately.
     blocked = q1["kernel"] == binding.KERNEL_BLOCKED
+    stream_k = q1["kernel"] == binding.KERNEL_STREAM
     launch_us = ms_main * 1e3 / max(n_main, 1) if n_main else ms_local * 1e3 / max(launches, 1)
     b_survey = sum(BYTES_SURVEY.values()) * nvox_all
     b_build = sum(BYTES_BUILD.values()) * nvox_all
     achieved = b_survey / (launch_us * 1e-6) / 1e9
-    vkey = variant_key(w.name, variant) if blocked else f"{w.name}/plain"
+    vkey = variant_key(w.name, variant) + ("/tma" if stream_k else "") if (blocked or stream_k) else f"{w.name}/plain"
     traffic, traffic_src = NCU_TRAFFIC.get(vkey, (None, None))
     roofline = {
         # S = 1: one pass over the field per step, the HBM stream binds.  S >= 2: the kernel moves the same bytes per
         # launch but does S steps of arithmetic on them; ncu shows the issue slots, not DRAM, as the busiest unit
         # (profiles/): frac stays the true share of the HBM peak, it is just not what limits the kernel
-        "bound": "hbm" if (not blocked or S == 1) else "issue",
+        "bound": "hbm" if (not blocked or S == 1) else "issue",      # (the one-step kernels, blocked S = 1 or TMA-staged: HBM)
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "traffic": traffic, "traffic_source": traffic_src, "variant": vkey, "peak_source": peak_src,
-        "kernel": f"rfa_blocked_kernel<S={S}>" if blocked else "rfa_plain_kernel",
+        "kernel": f"rfa_blocked_kernel<S={S}>" if blocked else ("rfa_stream_kernel (TMA, S=1)" if stream_k else "rfa_plain_kernel"),
         "launches": launches, "full_launches": n_main, "avg_launch_us": launch_us,
         "remainder_launch": {"steps": k_rem, "us": (ms_local - ms_main) * 1e3} if k_rem else None,
         "algorithmic_bytes_per_launch": b_survey, "bytes_per_voxel": BYTES_SURVEY,
@@ -576,7 +577,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=120)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5", "C4F"])
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 plain, 2 blocked (rfa_configure)")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 plain, 2 blocked, 3 TMA-staged one-step (rfa_configure)")
     ap.add_argument("--fused", type=int, default=0, help="fused time steps per launch, 0 = library default")
     ap.add_argument("--conduction", default="eq12", choices=["eq12", "face"],
                     help="eq12: Eq. 12 as printed (default, the headline); face: conservative div(K grad T), row f1")

@@ -82,7 +82,11 @@ enum {
 enum {
     RFA_KERNEL_AUTO = 0,      /* temporally blocked kernel where the grid allows it, else the plain one */
     RFA_KERNEL_PLAIN = 1,     /* one thread per voxel, one step per launch, global loads only          */
-    RFA_KERNEL_BLOCKED = 2    /* 2.5D z-sweep with register queues, fused_steps time steps per launch   */
+    RFA_KERNEL_BLOCKED = 2,   /* 2.5D z-sweep with register queues, fused_steps time steps per launch   */
+    RFA_KERNEL_STREAM = 3     /* one time step per launch (the frame loop of Alg. 2), 128 x 32 tiles with
+                                 halos staged in shared memory by the Tensor Memory Accelerator; needs nx % 16 == 0 and
+                                 RFA_COND_EQ12.  RFA_KERNEL_AUTO uses it for every single-step launch where it applies
+                                 (fused_steps = 1, and the remainder launch of n % fused_steps = 1)               */
 };
 
 /* Bytes of device workspace rfa_create needs for these dims (nx,ny,nz) and batch; 0 on bad input. */
@@ -137,7 +141,8 @@ int rfa_get_necrosis(rfa_sim *s, int scenario, uint8_t *out);
  * voxels nor held labels (the reported necrotic volume, R-13).  Either pointer may be NULL. */
 int rfa_necrotic_voxels(rfa_sim *s, int scenario, int64_t *all_voxels, int64_t *tissue_voxels);
 
-/* Choose the kernel variant and, for the blocked kernel, the number of fused time steps (1..4; 0 = default). */
+/* Choose the kernel variant and, for the blocked kernel, the number of fused time steps (1..4; 0 = default).
+ * RFA_KERNEL_STREAM takes fused_steps 0 or 1 and is rejected (RFA_E_INVALID) where it does not apply. */
 int rfa_configure(rfa_sim *s, int kernel, int fused_steps);
 
 /* Choose the conduction term for all scenarios (RFA_COND_*).  RFA_COND_FACE re-checks the monotone bound with

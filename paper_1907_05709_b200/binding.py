@@ -17,7 +17,7 @@ LIB_PATH = os.environ.get("RFA_LIBRARY") or os.path.join(_HERE, "librfa.so")
 
 RFA_OK, RFA_E_INVALID, RFA_E_UNSTABLE, RFA_E_CUDA, RFA_E_NOMEM = 0, -1, -2, -3, -4
 SRC_OFF, SRC_DIRICHLET, SRC_POWER = 0, 1, 2
-KERNEL_AUTO, KERNEL_PLAIN, KERNEL_BLOCKED = 0, 1, 2
+KERNEL_AUTO, KERNEL_PLAIN, KERNEL_BLOCKED, KERNEL_STREAM = 0, 1, 2, 3
 TISSUE_HELD = 1
 MAX_TISSUES = 16
 COND_EQ12, COND_FACE = 0, 1

@@ -7,8 +7,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librfa.so")
-SOURCES = ["rfa_kernels.cu", "rfa_api.cpp"]
-HEADERS = ["rfa_device.cuh", "rfa_internal.h", os.path.join("..", "..", "include", "rfa.h")]
+SOURCES = ["rfa_kernels.cu", "rfa_stream.cu", "rfa_api.cpp"]
+HEADERS = ["rfa_device.cuh", "rfa_packed.cuh", "rfa_internal.h", os.path.join("..", "..", "include", "rfa.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

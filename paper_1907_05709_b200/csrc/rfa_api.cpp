@@ -58,8 +58,9 @@ struct rfa_sim {
     unsigned long long *counters = nullptr;
     int kernel = RFA_KERNEL_AUTO;
     int fused = 3;
-    RfaTbPlan plans[5]{};                // index = fused steps 1..4
-    int resident[5][RFA_N_SHAPES]{};
+    RfaTbPlan plans_by_mode[2][5]{};     // [conduction mode][fused steps 1..4]: the conservative variant needs more
+    int resident[2][5][RFA_N_SHAPES]{};  // shared memory (deeper state ring), so its occupancy and plan may differ
+    const RfaTbPlan *plans() const { return plans_by_mode[conduction == RFA_COND_FACE ? 1 : 0]; }
     long long launches = 0;
     long long *probes = nullptr;         // device, n_probes flat voxel indices (library-owned)
     int n_probes = 0;
@@ -67,6 +68,11 @@ struct rfa_sim {
     size_t record_cap = 0;               // floats
     float *stage = nullptr;              // device staging of host displacement fields / host images (library-owned,
     size_t stage_cap = 0;                // grows on demand; floats)
+    RfaTensorMap tm_theta[2]{};          // tensor maps of the two temperature images and of the state volume (TMA-staged
+    RfaTensorMap tm_state{};             // one-step kernel, rfa_stream.cu)
+    bool stream_ok = false;              // the grid has a TMA path (nx % 16 == 0, driver entry point found)
+    RfaTbPlan stream_plan{};
+    unsigned long long stream_draws = 0; // items drawn so far from the dynamic work counter (counters[4]; never reset)
     int device = 0;                      // the CUDA device the simulation lives on (current device at rfa_create)
     int held_copy_auto = 0;              // what rfa_create chose for the held-copy variant (RFA_HELD_COPY_AUTO)
 };
@@ -264,6 +270,40 @@ RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const i
     return best;
 }
 
+// Plan of the TMA-staged one-step kernel: 128 x 16 tiles without redundant voxels (the halo is loaded, not computed).  The
+// work items (tile x z chunk) are handed out dynamically, so the chunk length trades the two neighbour planes every
+// chunk streams on top of its own against the tail of the last round: cost = planes per CTA + one item (measured on the
+// B200, C4: 8 / 12 / 16 / 22 / 32 chunks -> 114 / 111 / 109 / 113 / 119 us per step).
+RfaTbPlan rfa_plan_stream(int nx, int ny, int nz, int batch, int resident_ctas)
+{
+    RfaTbPlan p{};
+    p.fused = 1;
+    if (resident_ctas < 1 || nx < 1 || ny < 1 || nz < 1 || batch < 1 || (nx % 16) != 0) return p;
+    if ((long long)(nx / 4) * ny * nz >= 0x7fffffffLL) return p;
+    p.tiles_x = (nx + RFA_STREAM_BX - 1) / RFA_STREAM_BX;
+    p.tiles_y = (ny + RFA_STREAM_BY - 1) / RFA_STREAM_BY;
+    const long long per_z = (long long)p.tiles_x * p.tiles_y * batch;
+    double best = 1e300;
+    for (int nzc = 1; nzc <= nz; ++nzc) {
+        const int zchunk = (nz + nzc - 1) / nzc;
+        if ((nzc - 1) * zchunk >= nz) continue;
+        const long long items = per_z * nzc;
+        const double item_planes = zchunk + 3;                   // two neighbour planes + pipeline refill
+        const double cost = (double)items * item_planes / resident_ctas + item_planes;
+        if (cost < best - 1e-9) {
+            best = cost;
+            p.nzc = nzc;
+            p.zchunk = zchunk;
+        }
+    }
+    const long long items = per_z * p.nzc;
+    if (p.nzc < 1 || items > 0x7fffffffLL) return p;
+    p.n_items = (int)items;
+    p.grid = (int)std::min<long long>(items, resident_ctas);
+    p.ok = 1;
+    return p;
+}
+
 // exported for the CPU unit tests of the planner (no GPU needed)
 extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resident_ctas, int out[9])
 {
@@ -317,15 +357,21 @@ static int upload_table(rfa_sim *s, int scenario)
 // level expensive (10 useful rows of 16 at S = 3, 12 at S = 2; measured on the 128^3 volumes: 696 vs 670 GVox/s).
 static int default_fused(const rfa_sim *s)
 {
-    if (s->plans[3].ok && s->plans[3].shape == 1 && s->plans[2].ok) return 2;
+    if (s->plans()[3].ok && s->plans()[3].shape == 1 && s->plans()[2].ok) return 2;
     return 3;
 }
 
 static void make_plans(rfa_sim *s)
 {
+    s->stream_ok = rfa_stream_make_maps(s->g, s->theta[0], s->state, &s->tm_theta[0], &s->tm_state) &&
+                   rfa_stream_make_maps(s->g, s->theta[1], nullptr, &s->tm_theta[1], nullptr);
+    s->stream_plan = s->stream_ok ? rfa_plan_stream(s->g.nx, s->g.ny, s->g.nz, s->g.batch, rfa_stream_resident_ctas()) : RfaTbPlan{};
+    if (!s->stream_plan.ok) s->stream_ok = false;
     for (int f = 1; f <= 4; ++f) {
-        for (int sh = 0; sh < RFA_N_SHAPES; ++sh) s->resident[f][sh] = rfa_blocked_resident_ctas(f, sh);
-        s->plans[f] = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, s->resident[f]);
+        for (int m = 0; m < 2; ++m) {
+            for (int sh = 0; sh < RFA_N_SHAPES; ++sh) s->resident[m][f][sh] = rfa_blocked_resident_ctas(f, sh, m);
+            s->plans_by_mode[m][f] = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, s->resident[m][f]);
+        }
     }
 }
 
@@ -471,6 +517,8 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     int rc = RFA_OK;
     do {
         // labels -> device (staged through scratch), then label -> initial temperature image
+        e = cudaMemsetAsync(s->counters, 0, 256, s->stream);   // necrotic-voxel counts [0..1], dynamic work counter [4]
+        if (e != cudaSuccess) { rc = cuda_fail(e, "counter reset"); break; }
         e = cudaMemcpyAsync(s->scratch, labels, nvox, cudaMemcpyHostToDevice, s->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "label upload"); break; }
         float theta0[RFA_NLABEL], kl[RFA_NLABEL], kap[RFA_NLABEL * RFA_NLABEL];
@@ -597,13 +645,32 @@ extern "C" int rfa_set_temperature(rfa_sim *s, int scenario, const float *t_c)
     return RFA_OK;
 }
 
+// the TMA-staged one-step kernel serves single-step launches in Eq. 12 mode on grids with a TMA path
+static bool can_stream(const rfa_sim *s) { return s->stream_ok && s->conduction == RFA_COND_EQ12; }
+
+// what a launch of `did` time steps runs, given the configured kernel
+static int kernel_for(const rfa_sim *s, int did)
+{
+    if (s->kernel == RFA_KERNEL_PLAIN) return RFA_KERNEL_PLAIN;
+    if (did == 1 && can_stream(s) && (s->kernel == RFA_KERNEL_AUTO || s->kernel == RFA_KERNEL_STREAM)) return RFA_KERNEL_STREAM;
+    if (s->kernel == RFA_KERNEL_STREAM) return s->plans()[1].ok ? RFA_KERNEL_BLOCKED : RFA_KERNEL_PLAIN;   // e.g. after rfa_set_conduction
+    return s->plans()[did].ok ? RFA_KERNEL_BLOCKED : RFA_KERNEL_PLAIN;
+}
+
 extern "C" int rfa_configure(rfa_sim *s, int kernel, int fused_steps)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
-    if (kernel != RFA_KERNEL_AUTO && kernel != RFA_KERNEL_PLAIN && kernel != RFA_KERNEL_BLOCKED) return fail(RFA_E_INVALID, "bad kernel id %d", kernel);
+    if (kernel != RFA_KERNEL_AUTO && kernel != RFA_KERNEL_PLAIN && kernel != RFA_KERNEL_BLOCKED && kernel != RFA_KERNEL_STREAM)
+        return fail(RFA_E_INVALID, "bad kernel id %d", kernel);
     if (fused_steps < 0 || fused_steps > 4) return fail(RFA_E_INVALID, "fused_steps must be 0..4");
-    const int f = fused_steps == 0 ? default_fused(s) : fused_steps;
-    if (kernel == RFA_KERNEL_BLOCKED && !s->plans[f].ok)
+    int f = fused_steps == 0 ? default_fused(s) : fused_steps;
+    if (kernel == RFA_KERNEL_STREAM) {
+        if (!can_stream(s))
+            return fail(RFA_E_INVALID, "the TMA-staged one-step kernel needs nx %% 16 == 0 and the Eq. 12 conduction term (grid %dx%dx%d)", s->g.nx, s->g.ny, s->g.nz);
+        if (fused_steps > 1) return fail(RFA_E_INVALID, "the one-step kernel takes fused_steps 0 or 1");
+        f = 1;
+    }
+    if (kernel == RFA_KERNEL_BLOCKED && !s->plans()[f].ok)
         return fail(RFA_E_INVALID, "the blocked kernel needs nx %% 4 == 0 and ny, nz >= fused steps (grid %dx%dx%d, fused %d)", s->g.nx, s->g.ny, s->g.nz, f);
     s->kernel = kernel;
     s->fused = f;
@@ -643,9 +710,9 @@ extern "C" int rfa_set_conduction(rfa_sim *s, int mode)
 extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launches)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
-    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
-    if (kernel) *kernel = blocked ? RFA_KERNEL_BLOCKED : RFA_KERNEL_PLAIN;
-    if (fused_steps) *fused_steps = blocked ? s->fused : 1;
+    const int k = kernel_for(s, s->fused);
+    if (kernel) *kernel = k;
+    if (fused_steps) *fused_steps = k == RFA_KERNEL_BLOCKED ? s->fused : 1;
     if (kernel_launches) *kernel_launches = s->launches;
     return RFA_OK;
 }
@@ -654,18 +721,26 @@ extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *ker
 static int advance(rfa_sim *s, int n)
 {
     const float *kap = s->conduction == RFA_COND_FACE ? s->kap : nullptr;
-    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
+    const int fused = (s->kernel == RFA_KERNEL_PLAIN || s->kernel == RFA_KERNEL_STREAM) ? 1 : s->fused;
     while (n > 0) {
         cudaError_t e;
-        int did = 1;
-        if (blocked) {
-            did = std::min(n, s->fused);
-            while (did > 1 && !s->plans[did].ok) --did;
+        int did = std::min(n, fused);
+        while (did > 1 && !s->plans()[did].ok) --did;
+        const int k = kernel_for(s, did);
+        float *tin = s->theta[s->cur], *tout = s->theta[s->cur ^ 1];
+        unsigned char *rin = s->resid[s->cur], *rout = s->resid[s->cur ^ 1];
+        if (k == RFA_KERNEL_STREAM)
+        {
+            e = rfa_launch_stream(s->g, s->stream_plan, s->tm_theta[s->cur], s->tm_state, tout, rin, rout, s->state, s->tables,
+                                  s->counters + 4, s->stream_draws, s->stream);
+            s->stream_draws += (unsigned long long)s->stream_plan.n_items;   // every launch draws exactly n_items times
         }
-        if (blocked && s->plans[did].ok)
-            e = rfa_launch_blocked(s->g, s->plans[did], s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, kap, s->stream);
-        else
-            e = rfa_launch_plain(s->g, s->theta[s->cur], s->theta[s->cur ^ 1], s->resid[s->cur], s->resid[s->cur ^ 1], s->state, s->tables, kap, s->stream);
+        else if (k == RFA_KERNEL_BLOCKED)
+            e = rfa_launch_blocked(s->g, s->plans()[did], tin, tout, rin, rout, s->state, s->tables, kap, s->stream);
+        else {
+            did = 1;
+            e = rfa_launch_plain(s->g, tin, tout, rin, rout, s->state, s->tables, kap, s->stream);
+        }
         s->launches++;
         if (e != cudaSuccess) return cuda_fail(e, "step kernel");
         s->cur ^= 1;                                        // Alg. 2: swap the two buffers
@@ -677,13 +752,14 @@ static int advance(rfa_sim *s, int n)
 extern "C" int rfa_query_variant(rfa_sim *s, int out[6])
 {
     if (!s || !out) return fail(RFA_E_INVALID, "null argument");
-    const bool blocked = s->kernel != RFA_KERNEL_PLAIN && s->plans[s->fused].ok;
-    const RfaTbPlan &p = s->plans[s->fused];
+    const int k = kernel_for(s, s->fused);
+    const RfaTbPlan &p = s->plans()[s->fused];
+    const bool blocked = k == RFA_KERNEL_BLOCKED, stream = k == RFA_KERNEL_STREAM;
     out[0] = blocked ? s->fused : 1;
-    out[1] = blocked ? 4 * RFA_TB_SHAPE[p.shape][s->fused].tx : 0;
-    out[2] = blocked ? RFA_TB_SHAPE[p.shape][s->fused].ry * RFA_TB_SHAPE[p.shape][s->fused].ty : 0;
-    out[3] = blocked ? p.grid : 0;
-    out[4] = blocked ? s->g.held_copy : 0;
+    out[1] = blocked ? 4 * RFA_TB_SHAPE[p.shape][s->fused].tx : (stream ? RFA_STREAM_BX : 0);
+    out[2] = blocked ? RFA_TB_SHAPE[p.shape][s->fused].ry * RFA_TB_SHAPE[p.shape][s->fused].ty : (stream ? RFA_STREAM_BY : 0);
+    out[3] = blocked ? p.grid : (stream ? s->stream_plan.grid : 0);
+    out[4] = (blocked || stream) ? s->g.held_copy : 0;
     out[5] = s->conduction;
     return RFA_OK;
 }

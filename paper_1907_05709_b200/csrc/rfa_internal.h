@@ -110,5 +110,39 @@ cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, co
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
                                const void *rin, void *rout, uint8_t *state, const float *tables, const float *kap,
                                cudaStream_t st);
-// resident CTAs of the blocked kernel on the current device for `fused` steps (occupancy * SM count)
-int rfa_blocked_resident_ctas(int fused, int shape);
+// ---- one-step kernel staged by the Tensor Memory Accelerator (rfa_stream.cu) ----------------------------------------
+// tile of one CTA: RFA_STREAM_BX x RFA_STREAM_BY voxels (8 warps x RFA_STREAM_RY rows, one float4 column per lane), a ring of
+// RFA_STREAM_D shared-memory slots per CTA (D - 2 planes in flight).  Measured on the B200 (C4, us per step): 2 rows per
+// warp 146, 4 rows 198-241, 1 row with 16 warps 152; ring depth 3 / 4 / 6 / 8: 164 / 152 / 163 / 168; 3 or 4 CTAs per SM
+// 186-204: this memory system wants about two planes in flight per CTA and few concurrent streams, not more of either.
+#define RFA_STREAM_BX 128
+#ifndef RFA_STREAM_RY
+#define RFA_STREAM_RY 2
+#endif
+#ifndef RFA_STREAM_NW
+#define RFA_STREAM_NW 8                    // warps per CTA, each owning RFA_STREAM_RY rows of the tile
+#endif
+#define RFA_STREAM_BY (RFA_STREAM_NW * RFA_STREAM_RY)
+#ifndef RFA_STREAM_D
+#define RFA_STREAM_D 4
+#endif
+#ifndef RFA_STREAM_MINB
+#define RFA_STREAM_MINB 2                  // CTAs per SM asked of the compiler (register cap)
+#endif
+struct alignas(64) RfaTensorMap {
+    unsigned long long opaque[16];   // a CUtensorMap (cuda.h), kept opaque so that host code needs no driver header
+};
+// tensor maps of one fp32 image / of the packed state volume, both seen as (nx, ny, nz * batch); either output may be null.
+// false: no TMA path for this grid (nx % 16 != 0) or no driver entry point
+bool rfa_stream_make_maps(const RfaGrid &g, const float *theta, const uint8_t *state, RfaTensorMap *map_theta, RfaTensorMap *map_state);
+int rfa_stream_resident_ctas();
+// plan fields used: tiles_x, tiles_y, nzc, zchunk, n_items, grid
+RfaTbPlan rfa_plan_stream(int nx, int ny, int nz, int batch, int resident_ctas);
+cudaError_t rfa_launch_stream(const RfaGrid &g, const RfaTbPlan &plan, const RfaTensorMap &map_theta_in, const RfaTensorMap &map_state,
+                              float *tout, const void *rin, void *rout, uint8_t *state, const float *tables,
+                              unsigned long long *work_ctr /*device, never reset*/, unsigned long long work_base /*its value at launch*/,
+                              cudaStream_t st);
+
+// resident CTAs of the blocked kernel on the current device for `fused` steps (occupancy * SM count);
+// cons = 1: the conservative-conduction variant
+int rfa_blocked_resident_ctas(int fused, int shape, int cons);

@@ -358,8 +358,12 @@ struct TbCfg {
     static constexpr int NT = TX * TY;
     static constexpr int BX = 4 * TX;
     static constexpr int BY = RY * TY;
-    static constexpr int PD = 1;                                  // prefetch distance (planes in flight)
-    static constexpr int DT = 2;                                  // temperature ring depth (PD + 1)
+#ifndef RFA_S1_PD
+#define RFA_S1_PD 1
+#endif
+    // prefetch distance (planes in flight): the one-step kernel is bound by memory latency, not by issue slots
+    static constexpr int PD = S == 1 ? RFA_S1_PD : 1;
+    static constexpr int DT = rfa_pow2_at_least(PD + 1);          // temperature ring depth
     // state ring depth: level k reads plane i-k-1; the conservative mode also reads the planes i-k and i-k-2 and
     // the rows of the neighbouring threads (one extra slot keeps a thread one barrier ahead off them)
     static constexpr int DS = rfa_pow2_at_least(CONS ? PD + S + 3 : PD + S + 1);
@@ -367,49 +371,14 @@ struct TbCfg {
     static constexpr size_t RING_T = (size_t)DT * RY * NT * 16;
     static constexpr size_t EXCH = (size_t)S * 2 * 2 * NT * 16;
     static constexpr size_t RING_S = (size_t)DS * RY * NT * 4;
-    static constexpr size_t RSM = (size_t)NR * 2 * RY * NT * 8;
+    static constexpr size_t RSM = S > 1 ? (size_t)NR * 2 * RY * NT * 8 : 0;
     static constexpr size_t TAB = 3 * RFA_TABLE_N * 4;
     static constexpr size_t KAP = CONS ? RFA_NLABEL * RFA_NLABEL * 4 : 0;
     static constexpr size_t SMEM = RING_T + EXCH + RING_S + RSM + TAB + KAP;
 };
 
 #define RFA_MAX_DEVICES 64
-typedef unsigned long long u64;
-__device__ __forceinline__ u64 pk(float lo, float hi)
-{
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void upk(u64 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ u64 add2(u64 a, u64 b)
-{
-    u64 r;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
-{
-    u64 r;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-    return r;
-}
-__device__ __forceinline__ float max3abs(float a, float b, float c) { return fmaxf(fmaxf(fabsf(a), fabsf(b)), fabsf(c)); }
-__device__ __forceinline__ float max_abs4(const float4 v, float m) { return fmaxf(max3abs(v.x, v.y, v.z), fmaxf(fabsf(v.w), m)); }
-__device__ __forceinline__ uint2 pack_h4(float a, float b, float c, float d)
-{
-    const __half2 lo = __floats2half2_rn(a, b), hi = __floats2half2_rn(c, d);
-    uint2 r;
-    r.x = *reinterpret_cast<const unsigned *>(&lo);
-    r.y = *reinterpret_cast<const unsigned *>(&hi);
-    return r;
-}
-__device__ __forceinline__ float4 unpack_h4(const uint2 v)
-{
-    const float2 lo = __half22float2(*reinterpret_cast<const __half2 *>(&v.x));
-    const float2 hi = __half22float2(*reinterpret_cast<const __half2 *>(&v.y));
-    return make_float4(lo.x, lo.y, hi.x, hi.y);
-}
+#include "rfa_packed.cuh"
 
 // Conservative conduction, one row of four voxels (rfa_device.cuh: rfa_face_correction; R-28): g of
 // every voxel whose interface bit is set gets the face correction added.  w = the row's state word, w?? = the
@@ -601,6 +570,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
             float4 out[RY];
             uint2 rout[RY];
             unsigned nb_out = 0;
+            bool write_res = true;
 #pragma unroll
             for (int k = 0; k < S; ++k) {
                 // publish first/last row of the arriving level-k plane (it is the centre plane next iteration)
@@ -716,6 +686,10 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
 #pragma unroll
                     for (int r = 0; r < RY; ++r)
                         if (k + 1 == S) rout[r] = make_uint2(0u, 0u);
+                    // A residual is read only where |theta| >= RFA_COMP_MIN at the start of a step (rfa_advance), i.e. where
+                    // the output of the step before reaches it: rows that are cold before and after the last fused step
+                    // need no residual store (whatever the image holds there is never looked at)
+                    if (k + 1 == S) write_res = mx >= RFA_COMP_MIN;
                 } else {
                     // rfa_advance() in full, two voxels per instruction (o - t and d - bv as exact-product FMAs)
                     const u64 neg1 = pk(-1.0f, -1.0f), mg = pk(RFA_COMP_MAGIC, RFA_COMP_MAGIC), nmg = pk(-RFA_COMP_MAGIC, -RFA_COMP_MAGIC);
@@ -781,7 +755,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 for (int r = 0; r < RY; ++r) {
                     if (row_ok & (1u << r)) {
                         tout4[pl + row_dst[r]] = out[r];
-                        rout2[pl + row_dst[r]] = rout[r];
+                        if (write_res) rout2[pl + row_dst[r]] = rout[r];
                         const unsigned bits = (nb_out >> (4 * r)) & 0xfu;
                         if (bits) {
                             const uint32_t w = ringS[(sS * NT + tid) * RY + r];
@@ -1020,10 +994,10 @@ cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const fl
     }
 }
 
-template <int S, int SHAPE>
+template <int S, int SHAPE, bool CONS>
 static int resident_s()
 {
-    using K = TbKernel<S, true, SHAPE>;     // the conservative variant needs the larger state ring: plan for it
+    using K = TbKernel<S, CONS, SHAPE>;
     auto kern = K::get();
     int dev = 0, sms = 0, occ = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;
@@ -1038,22 +1012,20 @@ static int resident_s()
     return sms * occ;
 }
 
-int rfa_blocked_resident_ctas(int fused, int shape)
+template <int S>
+static int resident_sc(int shape, int cons)
 {
-    if (shape == 0) {
-        switch (fused) {
-        case 1: return resident_s<1, 0>();
-        case 2: return resident_s<2, 0>();
-        case 3: return resident_s<3, 0>();
-        case 4: return resident_s<4, 0>();
-        default: return 0;
-        }
-    }
+    if (shape == 0) return cons ? resident_s<S, 0, true>() : resident_s<S, 0, false>();
+    return cons ? resident_s<S, 1, true>() : resident_s<S, 1, false>();
+}
+
+int rfa_blocked_resident_ctas(int fused, int shape, int cons)
+{
     switch (fused) {
-    case 1: return resident_s<1, 1>();
-    case 2: return resident_s<2, 1>();
-    case 3: return resident_s<3, 1>();
-    case 4: return resident_s<4, 1>();
+    case 1: return resident_sc<1>(shape, cons);
+    case 2: return resident_sc<2>(shape, cons);
+    case 3: return resident_sc<3>(shape, cons);
+    case 4: return resident_sc<4>(shape, cons);
     default: return 0;
     }
 }

@@ -88,6 +88,60 @@ def test_ragged_parity_and_variants(rfa, oracle, case):
             rfa.from_workload(w).configure(rfa.KERNEL_BLOCKED, 2)
 
 
+STREAM_CASES = [
+    dict(dims=(144, 70, 21), spacing=(0.7, 0.9, 1.3), steps=37, mode=W.SRC_DIRICHLET, value=90.0, batch=1),   # 2 x 3 tiles, ragged
+    dict(dims=(80, 130, 19), spacing=(1.1, 0.8, 0.9), steps=41, mode=W.SRC_POWER, value=2.0e7, batch=1),       # partial x tile
+    dict(dims=(16, 38, 29), spacing=(1.0, 1.0, 1.0), steps=50, mode=W.SRC_DIRICHLET, value=60.0, batch=1),     # narrower than a tile
+    dict(dims=(272, 33, 5), spacing=(0.7, 0.9, 1.3), steps=20, mode=W.SRC_DIRICHLET, value=90.0, batch=1),     # 3 x tiles, 1-row tail
+    dict(dims=(64, 66, 23), spacing=(1.0, 1.0, 1.2), steps=33, mode=W.SRC_DIRICHLET, value=90.0, batch=5),     # batched
+]
+
+
+@pytest.mark.parametrize("case", STREAM_CASES, ids=lambda c: "x".join(map(str, c["dims"])) + f"b{c['batch']}")
+def test_stream_kernel_parity_and_bit_identity(rfa, oracle, case):
+    """The TMA-staged one-step kernel (RFA_KERNEL_STREAM: cp.async.bulk.tensor tiles with halos, mbarrier ring) against the
+    oracle and, bit for bit, against the plain kernel; both held-copy settings; also as the remainder launch of S = 3."""
+    w = W.ragged_phantom(dims=case["dims"], spacing=case["spacing"], steps=case["steps"], mode=case["mode"],
+                         value=case["value"], q_m=10714.0, dt=0.05, batch=case["batch"])
+    w.table["t_init"][W.KIDNEY] = 36.0
+    Tp, Np, qp = run_gpu(rfa, w, w.steps, rfa.KERNEL_PLAIN)
+    for hc in (0, 1):
+        sim = rfa.from_workload(w)
+        sim.configure(rfa.KERNEL_STREAM, 1)
+        sim.configure_held_copy(hc)
+        q = sim.query()
+        assert q["kernel"] == rfa.KERNEL_STREAM and q["fused_steps"] == 1
+        v = sim.query_variant()
+        assert (v["tile_bx"], v["tile_by"], v["held_copy"]) == (128, 16, hc)
+        sim.step(w.steps)
+        for b in range(w.batch):
+            T, N = sim.get_temperature(b), sim.get_necrosis(b)
+            assert np.array_equal(T.view(np.uint32), Tp[b].view(np.uint32)), f"stream kernel differs from plain (scenario {b}, hc {hc})"
+            assert np.array_equal(N, Np[b])
+        sim.close()
+    for b in range(w.batch):
+        compare(Tp[b], Np[b], oracle.run_workload(w, scenario=b))
+    # default configuration: launches of 3 fused steps, a remainder of ONE step goes to the one-step kernel
+    if w.steps % 3 == 1:
+        Ta, Na, qa = run_gpu(rfa, w, w.steps, rfa.KERNEL_AUTO, 3)
+        assert np.array_equal(Ta[0].view(np.uint32), Tp[0].view(np.uint32)) and np.array_equal(Na[0], Np[0])
+    # not available: nx % 16 != 0, conservative conduction
+    w2 = W.ragged_phantom(dims=(136, 70, 21), steps=3)
+    sim = rfa.from_workload(w2)
+    with pytest.raises(rfa.RfaError):
+        sim.configure(rfa.KERNEL_STREAM, 1)
+    sim.configure(rfa.KERNEL_AUTO, 1)
+    assert sim.query()["kernel"] == rfa.KERNEL_BLOCKED
+    sim.close()
+    sim = rfa.from_workload(w)
+    sim.set_conduction(rfa.COND_FACE)
+    with pytest.raises(rfa.RfaError):
+        sim.configure(rfa.KERNEL_STREAM, 1)
+    sim.configure(rfa.KERNEL_AUTO, 1)
+    assert sim.query()["kernel"] == rfa.KERNEL_BLOCKED
+    sim.close()
+
+
 def test_batched_scenarios(rfa, oracle):
     w = W.ragged_phantom(dims=(68, 66, 23), spacing=(1.0, 1.0, 1.2), steps=33, batch=5, dt=0.08)
     T, N, q = run_gpu(rfa, w, w.steps, rfa.KERNEL_BLOCKED, 2)
@@ -698,14 +752,15 @@ def test_c5_sweep_fieldwide_vs_live_oracle(rfa, oracle):
 @pytest.mark.parametrize("name", ["C4", "C3"])
 def test_full_size_variants_bit_identical_fieldwide(rfa, name):
     """C4 / C3 with a smooth non-uniform start (every voxel changes every step): 30 steps of the plain kernel
-    (one thread per voxel, no tiles) against the blocked kernel with S = 1, 2, 3 fused steps in both held-copy
-    settings, the whole field bit for bit.  This is what exercises all work items of the full-size plan
+    (one thread per voxel, no tiles) against the blocked kernel with S = 1, 2, 3 fused steps and the TMA-staged
+    one-step kernel, each in both held-copy settings, the whole field bit for bit.  This is what exercises all work items of the full-size plan
     (C4: 540 items on 296 CTAs, the multi-item-per-CTA loop) in Eq. 12 mode."""
     w = W.with_smooth_field(W.BENCH_CONFIGS[name](steps=30))
     ref = None
     for kernel, fused, hc in [(rfa.KERNEL_PLAIN, 0, 0), (rfa.KERNEL_BLOCKED, 3, 1), (rfa.KERNEL_BLOCKED, 3, 0),
                               (rfa.KERNEL_BLOCKED, 2, 1), (rfa.KERNEL_BLOCKED, 2, 0), (rfa.KERNEL_BLOCKED, 1, 1),
-                              (rfa.KERNEL_BLOCKED, 1, 0), (rfa.KERNEL_BLOCKED, 4, 1)]:
+                              (rfa.KERNEL_BLOCKED, 1, 0), (rfa.KERNEL_BLOCKED, 4, 1), (rfa.KERNEL_STREAM, 1, 1),
+                              (rfa.KERNEL_STREAM, 1, 0)]:
         sim = rfa.from_workload(w)
         sim.configure(kernel, fused)
         sim.configure_held_copy(hc)
