@@ -1,35 +1,50 @@
-"""Builds librfa.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a."""
+"""Builds librfa.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+Every source is compiled to its own object (in parallel, only when it or a header is newer), then linked."""
 from __future__ import annotations
 
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librfa.so")
-SOURCES = ["rfa_kernels.cu", "rfa_stream.cu", "rfa_api.cpp"]
+SOURCES = ["rfa_kernels.cu", "rfa_stream.cu", "rfa_view.cu", "rfa_api.cpp"]
 HEADERS = ["rfa_device.cuh", "rfa_packed.cuh", "rfa_internal.h", os.path.join("..", "..", "include", "rfa.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-x", "cu", "--fmad=false",
+    "-Xcompiler", "-fPIC", "-x", "cu", "--fmad=false",
 ]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+def _newer_than(target: str, deps) -> bool:
+    if not os.path.exists(target):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    t = os.path.getmtime(target)
     return any(os.path.getmtime(d) > t for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a ... -> paper_1907_05709_b200/librfa.so"""
-    if force or _stale():
-        cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-              ["-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
-        subprocess.run(cmd, check=True)
+    os.makedirs(OBJ, exist_ok=True)
+    common = [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
+    jobs = []
+    for src in SOURCES:
+        obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+        if force or _newer_than(obj, [os.path.join(CSRC, src)] + common):
+            jobs.append(["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) +
+                        ["-c", "-o", obj, os.path.join(CSRC, src)])
+    if jobs:
+        with ThreadPoolExecutor(max_workers=len(jobs)) as ex:
+            for r in ex.map(lambda c: subprocess.run(c), jobs):
+                if r.returncode != 0:
+                    raise subprocess.CalledProcessError(r.returncode, r.args)
+    objs = [os.path.join(OBJ, os.path.splitext(s)[0] + ".o") for s in SOURCES]
+    if jobs or _newer_than(LIB, objs):
+        subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + objs, check=True)
     return LIB
 
 

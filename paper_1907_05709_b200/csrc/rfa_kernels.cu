@@ -129,105 +129,6 @@ __global__ void rfa_get_necrosis_kernel(size_t nvox, const uint8_t *__restrict__
     if (v < nvox) out[v] = state[v] >> 7;
 }
 
-// breathing-motion warp, Eq. 14: out[v] = T(x_v + scale * u[v]), trilinear, clamped (row f3).
-// The displacement is split into integer and fractional voxels BEFORE the voxel index is added, so the
-// interpolation weights keep the full fp32 resolution of the (small) displacement, not of the coordinate.
-// one axis of the sample position: the displacement d (in voxels) is clamped so that base + d stays inside
-// [0, n-1] (bounds exact in fp32: small integers), then split into cell index and weight.  d keeps its own fp32
-// resolution: it is never added to the coordinate in floating point.
-__device__ __forceinline__ void rfa_warp_axis(int base, int n, float d, int &i0, int &i1, float &a)
-{
-    const float dc = fminf(fmaxf(d, -(float)base), (float)(n - 1 - base));
-    const float f = floorf(dc);
-    a = dc - f;
-    i0 = base + (int)f;
-    i1 = min(i0 + 1, n - 1);
-}
-
-__device__ __forceinline__ float rfa_warp_voxel(int i, int j, int k, int nx, int ny, int nz, const float *__restrict__ theta,
-                                                float dx, float dy, float dz, float t_blood)
-{
-    int i0[3], i1[3];
-    float a[3];
-    rfa_warp_axis(i, nx, dx, i0[0], i1[0], a[0]);
-    rfa_warp_axis(j, ny, dy, i0[1], i1[1], a[1]);
-    rfa_warp_axis(k, nz, dz, i0[2], i1[2], a[2]);
-    const size_t sy = nx, sz = (size_t)nx * ny;
-    const float *z0 = theta + (size_t)i0[2] * sz, *z1 = theta + (size_t)i1[2] * sz;
-    const size_t r0 = (size_t)i0[1] * sy, r1 = (size_t)i1[1] * sy;
-    const float c000 = __ldg(z0 + r0 + i0[0]), c100 = __ldg(z0 + r0 + i1[0]), c010 = __ldg(z0 + r1 + i0[0]),
-                c110 = __ldg(z0 + r1 + i1[0]), c001 = __ldg(z1 + r0 + i0[0]), c101 = __ldg(z1 + r0 + i1[0]),
-                c011 = __ldg(z1 + r1 + i0[0]), c111 = __ldg(z1 + r1 + i1[0]);
-    const float x00 = fmaf(a[0], c100 - c000, c000), x10 = fmaf(a[0], c110 - c010, c010);
-    const float x01 = fmaf(a[0], c101 - c001, c001), x11 = fmaf(a[0], c111 - c011, c011);
-    const float y0 = fmaf(a[1], x10 - x00, x00), y1 = fmaf(a[1], x11 - x01, x01);
-    return fmaf(a[2], y1 - y0, y0) + t_blood;
-}
-
-// grid = (x blocks, ny, nz): no integer division per voxel; VEC = 4 voxels per thread along x with 16-byte loads of
-// the three displacement components and a 16-byte store (nx % 4 == 0), VEC = 1 for any nx
-template <int VEC>
-__global__ void rfa_warp_kernel(int nx, int ny, int nz, const float *__restrict__ theta, const float *__restrict__ disp,
-                                float scale, float ihx, float ihy, float ihz, float t_blood, float *__restrict__ out)
-{
-    const int i = (blockIdx.x * blockDim.x + threadIdx.x) * VEC;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
-    if (i >= nx || j >= ny) return;
-    const size_t nvox = (size_t)nx * ny * nz;
-    const size_t v = (size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * k);
-    const float sx = scale * ihx, sy_ = scale * ihy, sz_ = scale * ihz;       // mm -> voxels, scaled
-    if constexpr (VEC == 4) {
-        const float4 ux = *reinterpret_cast<const float4 *>(disp + v), uy = *reinterpret_cast<const float4 *>(disp + nvox + v),
-                     uz = *reinterpret_cast<const float4 *>(disp + 2 * nvox + v);
-        float4 o;
-        o.x = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, ux.x * sx, uy.x * sy_, uz.x * sz_, t_blood);
-        o.y = rfa_warp_voxel(i + 1, j, k, nx, ny, nz, theta, ux.y * sx, uy.y * sy_, uz.y * sz_, t_blood);
-        o.z = rfa_warp_voxel(i + 2, j, k, nx, ny, nz, theta, ux.z * sx, uy.z * sy_, uz.z * sz_, t_blood);
-        o.w = rfa_warp_voxel(i + 3, j, k, nx, ny, nz, theta, ux.w * sx, uy.w * sy_, uz.w * sz_, t_blood);
-        *reinterpret_cast<float4 *>(out + v) = o;
-    } else {
-        out[v] = rfa_warp_voxel(i, j, k, nx, ny, nz, theta, disp[v] * sx, disp[nvox + v] * sy_, disp[2 * nvox + v] * sz_, t_blood);
-    }
-}
-
-// headless view of the heat zone (row f4; Figs. 11-12): orthographic ray-march, one thread per pixel.
-// Ray positions are carried in fp64 (a coordinate of ~500 voxels in fp32 would cost 6e-5 voxel = 3e-3 C at the
-// needle's 53 C/voxel gradient); the interpolation itself is fp32 like the warp.
-__global__ void rfa_render_kernel(RfaRay ray, int nx, int ny, int nz, const float *__restrict__ theta, float t_blood,
-                                  float iso_theta, float *__restrict__ tmax, float *__restrict__ depth)
-{
-    const int px = blockIdx.x * blockDim.x + threadIdx.x, py = blockIdx.y * blockDim.y + threadIdx.y;
-    if (px >= ray.width || py >= ray.height) return;
-    const double u = (px - 0.5 * (ray.width - 1)) * ray.pixel, v = (py - 0.5 * (ray.height - 1)) * ray.pixel;
-    double o[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) o[c] = ray.c[c] + u * ray.e1[c] + v * ray.e2[c] - ray.R * ray.w[c];
-    const size_t sy = nx, sz = (size_t)nx * ny;
-    float best = -3.0e38f;
-    int first = -1;
-    for (int m = 0; m < ray.n_samples; ++m) {
-        const double t = m * ray.step;
-        const double qx = (o[0] + t * ray.w[0]) * ray.inv_h[0] - 0.5, qy = (o[1] + t * ray.w[1]) * ray.inv_h[1] - 0.5,
-                     qz = (o[2] + t * ray.w[2]) * ray.inv_h[2] - 0.5;
-        if (qx < 0.0 || qy < 0.0 || qz < 0.0 || qx > nx - 1.0 || qy > ny - 1.0 || qz > nz - 1.0) continue;
-        const int i0 = min((int)qx, max(nx - 2, 0)), j0 = min((int)qy, max(ny - 2, 0)), k0 = min((int)qz, max(nz - 2, 0));
-        const int i1 = min(i0 + 1, nx - 1), j1 = min(j0 + 1, ny - 1), k1 = min(k0 + 1, nz - 1);
-        const float ax = (float)(qx - i0), ay = (float)(qy - j0), az = (float)(qz - k0);
-        const float *z0 = theta + (size_t)k0 * sz, *z1 = theta + (size_t)k1 * sz;
-        const size_t r0 = (size_t)j0 * sy, r1 = (size_t)j1 * sy;
-        const float c000 = __ldg(z0 + r0 + i0), c100 = __ldg(z0 + r0 + i1), c010 = __ldg(z0 + r1 + i0), c110 = __ldg(z0 + r1 + i1);
-        const float c001 = __ldg(z1 + r0 + i0), c101 = __ldg(z1 + r0 + i1), c011 = __ldg(z1 + r1 + i0), c111 = __ldg(z1 + r1 + i1);
-        const float x00 = fmaf(ax, c100 - c000, c000), x10 = fmaf(ax, c110 - c010, c010);
-        const float x01 = fmaf(ax, c101 - c001, c001), x11 = fmaf(ax, c111 - c011, c011);
-        const float y0 = fmaf(ay, x10 - x00, x00), y1 = fmaf(ay, x11 - x01, x01);
-        const float th = fmaf(az, y1 - y0, y0);
-        best = fmaxf(best, th);
-        if (first < 0 && th >= iso_theta) first = m;
-    }
-    const size_t pix = (size_t)py * ray.width + px;
-    tmax[pix] = (best > -1.0e38f ? best : 0.f) + t_blood;
-    if (depth) depth[pix] = first >= 0 ? (float)(first * ray.step) : -1.0f;
-}
 
 // probe read-out (Fig. 6): T at n flat voxel indices of the batched volume
 __global__ void rfa_probe_kernel(int n, const long long *__restrict__ index, const float *__restrict__ theta,
@@ -868,31 +769,6 @@ cudaError_t rfa_launch_get_necrosis(const RfaGrid &g, int scenario, const uint8_
     return cudaGetLastError();
 }
 
-cudaError_t rfa_launch_warp(const RfaGrid &g, int scenario, const float *theta, const float *disp_dev, float scale,
-                            const float inv_h_mm[3], float *out_dev, cudaStream_t st)
-{
-    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    const float *th = theta + (size_t)scenario * nvox;
-    const bool vec = (g.nx % 4) == 0 && (((uintptr_t)disp_dev | (uintptr_t)out_dev) & 15) == 0;
-    if (g.ny > 65535 * 4 || g.nz > 65535) return cudaErrorInvalidValue;
-    const dim3 block(64, 4, 1);
-    const dim3 grid((unsigned)((g.nx + (vec ? 256 : 64) - 1) / (vec ? 256 : 64)), (unsigned)((g.ny + 3) / 4), (unsigned)g.nz);
-    if (vec)
-        rfa_warp_kernel<4><<<grid, block, 0, st>>>(g.nx, g.ny, g.nz, th, disp_dev, scale, inv_h_mm[0], inv_h_mm[1], inv_h_mm[2], g.t_blood, out_dev);
-    else
-        rfa_warp_kernel<1><<<grid, block, 0, st>>>(g.nx, g.ny, g.nz, th, disp_dev, scale, inv_h_mm[0], inv_h_mm[1], inv_h_mm[2], g.t_blood, out_dev);
-    return cudaGetLastError();
-}
-
-cudaError_t rfa_launch_render(const RfaGrid &g, int scenario, const RfaRay &ray, const float *theta, float iso_theta,
-                              float *tmax_dev, float *depth_dev, cudaStream_t st)
-{
-    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    const dim3 block(16, 8, 1), grid((unsigned)((ray.width + 15) / 16), (unsigned)((ray.height + 7) / 8), 1);
-    rfa_render_kernel<<<grid, block, 0, st>>>(ray, g.nx, g.ny, g.nz, theta + (size_t)scenario * nvox, g.t_blood, iso_theta,
-                                              tmax_dev, depth_dev);
-    return cudaGetLastError();
-}
 
 cudaError_t rfa_launch_probe(const RfaGrid &g, int n, const long long *index_dev, const float *theta, float *out_dev,
                              cudaStream_t st)
