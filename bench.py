@@ -268,6 +268,12 @@ def run_ours(args):
         sim.configure(args.kernel, args.fused)
         if hc_env in ("0", "1"):
             sim.configure_held_copy(int(hc_env))
+        if args.staging != "auto":
+            sim.configure_staging(binding.STAGING_TMA if args.staging == "tma" else binding.STAGING_CP_ASYNC)
+        if args.tile >= 0:
+            sim.configure_tile(args.tile)
+        if args.res_prefetch != "auto":
+            sim.configure_residual_prefetch(binding.RES_PREFETCH_ON if args.res_prefetch == "on" else binding.RES_PREFETCH_OFF)
         if args.conduction == "face":
             sim.set_conduction(binding.COND_FACE)
         sim.step(Wu)
@@ -299,6 +305,7 @@ def run_ours(args):
                 sim.step(30 * S)
                 sim.synchronize()
         variant = sim.query_variant()
+        variant.update(sim.hot_fraction())
         necro_all, necro_tissue = sim.necrotic_voxels(0)
         tmax = float(sim.get_temperature(0).max())
         sim.close()
@@ -317,7 +324,8 @@ def run_ours(args):
     b_survey = sum(BYTES_SURVEY.values()) * nvox_all
     b_build = sum(BYTES_BUILD.values()) * nvox_all
     achieved = b_survey / (launch_us * 1e-6) / 1e9
-    vkey = variant_key(w.name, variant) + ("/tma" if stream_k else "") if (blocked or stream_k) else f"{w.name}/plain"
+    vkey = (variant_key(w.name, variant) + ("/tma" if variant.get("staging") == binding.STAGING_TMA else "") +
+            ("/rpf" if variant.get("residual_prefetch") else "")) if (blocked or stream_k) else f"{w.name}/plain"
     traffic, traffic_src = NCU_TRAFFIC.get(vkey, (None, None))
     roofline = {
         # S = 1: one pass over the field per step, the HBM stream binds.  S >= 2: the kernel moves the same bytes per
@@ -583,6 +591,12 @@ def main(argv=None):
                     help="eq12: Eq. 12 as printed (default, the headline); face: conservative div(K grad T), row f1")
     ap.add_argument("--op", default="step", choices=["step", "warp", "render", "record"],
                     help="step: the time-stepping hot path (the headline); warp: the Eq. 14 motion warp (row f3)")
+    ap.add_argument("--staging", default="auto", choices=["auto", "tma", "cp_async"],
+                    help="A/B switch: how the blocked kernel stages its input planes (rfa_configure_staging)")
+    ap.add_argument("--res-prefetch", default="auto", choices=["auto", "on", "off"],
+                    help="A/B switch: residual-prefetch variant of the blocked kernel (rfa_configure_residual_prefetch)")
+    ap.add_argument("--tile", type=int, default=-1, choices=[-1, 0, 1],
+                    help="A/B switch: tile shape of the blocked kernel, 0 = 64x32, 1 = 128x16 (rfa_configure_tile)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args(argv)

@@ -154,21 +154,45 @@ int rfa_set_conduction(rfa_sim *s, int mode);
 int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *kernel_launches);
 
 /* The variant rfa_step launches for this simulation:
- * out = { fused_steps, tile_bx, tile_by, ctas_launched, held_copy, conduction }.  held_copy = 1: the kernel variant in
+ * out = { fused_steps, tile_bx, tile_by, ctas_launched, held_copy, conduction, staging (RFA_STAGING_CP_ASYNC / _TMA),
+ *         residual_prefetch (0 / 1: what the next launch takes) }.  held_copy = 1: the kernel variant in
  * which warps whose voxels are all held copy their rows instead of evaluating the bracket (Alg. 1's else-branch,
  * PAPER.md:313; bit-identical), chosen at rfa_create when at least 1/8 of the volume carries a held label
  * (rfa_configure_held_copy overrides, for A/B measurements).  Zeros for the plain kernel. */
-int rfa_query_variant(rfa_sim *s, int out[6]);
+int rfa_query_variant(rfa_sim *s, int out[8]);
 
 /* Force the held-copy kernel variant on or off, or hand the choice back to the library (what rfa_create decided
  * from the share of held labels).  All settings give bit-identical fields; the library reads no environment variable. */
 enum { RFA_HELD_COPY_AUTO = -1, RFA_HELD_COPY_OFF = 0, RFA_HELD_COPY_ON = 1 };
 int rfa_configure_held_copy(rfa_sim *s, int mode);
 
+/* How the temporally blocked kernel brings the planes of the input image and the state bytes into shared memory (load step
+ * of Alg. 1): per-thread cp.async, or one bulk tensor copy (Tensor Memory Accelerator) per tile plane issued by
+ * a single thread.  The TMA variant exists for 2 and 3 fused steps in RFA_COND_EQ12 mode on grids with nx % 16 == 0 and ny
+ * even; AUTO (the default) takes it where it measured faster (the 128 x 16 tile).  All settings give bit-identical fields.  Returns RFA_E_INVALID,
+ * leaving the setting unchanged, when RFA_STAGING_TMA is asked for a grid that has no such variant. */
+enum { RFA_STAGING_AUTO = -1, RFA_STAGING_CP_ASYNC = 0, RFA_STAGING_TMA = 1 };
+int rfa_configure_staging(rfa_sim *s, int mode);
+
+/* Residual-prefetch variant of the blocked kernel (2 and 3 fused steps): the fp16 residual rows (compensated accumulation,
+ * DESIGN.md section 5) of planes with |T - T_a| >= 1 C are fetched one plane ahead instead of where they are used.  It pays
+ * where a few percent or more of the volume is that warm and costs ~3 % where next to nothing is, so in AUTO (the default) the
+ * library switches it on and off from the share of such planes that the kernels count as they run (no synchronisation:
+ * the count is copied to pinned memory asynchronously and looked at when it has arrived).  All settings give bit-identical
+ * fields.  rfa_query_hot_fraction returns the last share seen and the variant in use (either pointer may be NULL). */
+enum { RFA_RES_PREFETCH_AUTO = -1, RFA_RES_PREFETCH_OFF = 0, RFA_RES_PREFETCH_ON = 1 };
+int rfa_configure_residual_prefetch(rfa_sim *s, int mode);
+int rfa_query_hot_fraction(rfa_sim *s, double *fraction, int *prefetch_on);
+
+/* Force the tile shape of the blocked kernel: 0 = 64 x 32 voxels (16 x 16 threads), 1 = 128 x 16 (32 x 8 threads), -1 = the
+ * planner's choice (the default).  For A/B measurements; all shapes give bit-identical fields.  RFA_E_INVALID, leaving the
+ * setting unchanged, if the shape cannot run the configured number of fused steps on this grid. */
+int rfa_configure_tile(rfa_sim *s, int shape);
+
 /* Host-only view of the blocked kernel's launch plan for a grid (no GPU needed; used by the unit tests
  * and the bench report).  resident_ctas = CTAs that can be co-resident (SM count x occupancy).
  * out = { ok, tiles_x, tiles_y, z_chunks, planes_per_chunk, work_items, ctas_launched, tile_bx, tile_by }. */
-int rfa_plan_query(const int dims[3], int batch, int fused_steps, int resident_ctas, int out[9]);
+int rfa_plan_query(const int dims[3], int batch, int fused_steps, int resident_ctas, int staging, int out[9]);
 
 /* ---- probe time series and frame hand-off ---------------------------------
  * The paper reads temperatures at probe points 2.5 mm and 5 mm from the tip over 120 s (PAPER.md:147,

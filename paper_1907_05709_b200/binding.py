@@ -22,12 +22,14 @@ TISSUE_HELD = 1
 MAX_TISSUES = 16
 COND_EQ12, COND_FACE = 0, 1
 HELD_COPY_AUTO, HELD_COPY_OFF, HELD_COPY_ON = -1, 0, 1
+STAGING_AUTO, STAGING_CP_ASYNC, STAGING_TMA = -1, 0, 1
+RES_PREFETCH_AUTO, RES_PREFETCH_OFF, RES_PREFETCH_ON = -1, 0, 1
 
 # every symbol include/rfa.h declares
 EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
-    "rfa_set_conduction", "rfa_query", "rfa_query_variant", "rfa_configure_held_copy", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
+    "rfa_set_conduction", "rfa_query", "rfa_query_variant", "rfa_configure_held_copy", "rfa_configure_staging", "rfa_configure_tile", "rfa_configure_residual_prefetch", "rfa_query_hot_fraction", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
     "rfa_warp_temperature", "rfa_render_zone",
     "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
@@ -96,7 +98,15 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_query_variant.restype = ctypes.c_int
     lib.rfa_configure_held_copy.argtypes = [vp, ctypes.c_int]
     lib.rfa_configure_held_copy.restype = ctypes.c_int
-    lib.rfa_plan_query.argtypes = [i3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
+    lib.rfa_configure_staging.argtypes = [vp, ctypes.c_int]
+    lib.rfa_configure_staging.restype = ctypes.c_int
+    lib.rfa_configure_residual_prefetch.argtypes = [vp, ctypes.c_int]
+    lib.rfa_configure_residual_prefetch.restype = ctypes.c_int
+    lib.rfa_query_hot_fraction.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)]
+    lib.rfa_query_hot_fraction.restype = ctypes.c_int
+    lib.rfa_configure_tile.argtypes = [vp, ctypes.c_int]
+    lib.rfa_configure_tile.restype = ctypes.c_int
+    lib.rfa_plan_query.argtypes = [i3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
     lib.rfa_plan_query.restype = ctypes.c_int
     lib.rfa_set_probes.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int64)]
     lib.rfa_set_probes.restype = ctypes.c_int
@@ -145,10 +155,10 @@ def stability_number(spacing_mm, table, dt) -> float:
     return float(lib.rfa_stability_number(_f3(spacing_mm), tissue_array(table), len(table), float(dt)))
 
 
-def plan_query(dims, batch, fused, resident_ctas) -> dict:
+def plan_query(dims, batch, fused, resident_ctas, staging: int = 0) -> dict:
     lib = load_library()
     out = (ctypes.c_int * 9)()
-    _check(lib.rfa_plan_query(_i3(dims), int(batch), int(fused), int(resident_ctas), out))
+    _check(lib.rfa_plan_query(_i3(dims), int(batch), int(fused), int(resident_ctas), int(staging), out))
     keys = ["ok", "tiles_x", "tiles_y", "z_chunks", "planes_per_chunk", "work_items", "ctas", "bx", "by"]
     return dict(zip(keys, [int(x) for x in out]))
 
@@ -243,6 +253,20 @@ class RfaSim:
     def configure_held_copy(self, mode: int = HELD_COPY_AUTO):
         _check(self._lib.rfa_configure_held_copy(self._handle, int(mode)))
 
+    def configure_staging(self, mode: int = STAGING_AUTO):
+        _check(self._lib.rfa_configure_staging(self._handle, int(mode)))
+
+    def configure_residual_prefetch(self, mode: int = RES_PREFETCH_AUTO):
+        _check(self._lib.rfa_configure_residual_prefetch(self._handle, int(mode)))
+
+    def hot_fraction(self) -> dict:
+        f, on = ctypes.c_double(), ctypes.c_int()
+        _check(self._lib.rfa_query_hot_fraction(self._handle, ctypes.byref(f), ctypes.byref(on)))
+        return {"hot_fraction": float(f.value), "residual_prefetch": int(on.value)}
+
+    def configure_tile(self, shape: int = -1):
+        _check(self._lib.rfa_configure_tile(self._handle, int(shape)))
+
     def set_conduction(self, mode: int):
         _check(self._lib.rfa_set_conduction(self._handle, int(mode)))
 
@@ -252,9 +276,10 @@ class RfaSim:
         return {"kernel": int(k.value), "fused_steps": int(f.value), "kernel_launches": int(n.value)}
 
     def query_variant(self) -> dict:
-        out = (ctypes.c_int * 6)()
+        out = (ctypes.c_int * 8)()
         _check(self._lib.rfa_query_variant(self._handle, out))
-        return dict(zip(["fused_steps", "tile_bx", "tile_by", "ctas", "held_copy", "conduction"], [int(x) for x in out]))
+        return dict(zip(["fused_steps", "tile_bx", "tile_by", "ctas", "held_copy", "conduction", "staging", "residual_prefetch"],
+                        [int(x) for x in out]))
 
     def set_probes(self, index):
         idx = np.ascontiguousarray(index, dtype=np.int64).reshape(-1)

@@ -73,6 +73,22 @@ struct rfa_sim {
     bool stream_ok = false;              // the grid has a TMA path (nx % 16 == 0, driver entry point found)
     RfaTbPlan stream_plan{};
     unsigned long long stream_draws = 0; // items drawn so far from the dynamic work counter (counters[4]; never reset)
+    RfaTensorMap tm_blk_theta[2][RFA_N_SHAPES]{};   // blocked kernel, TMA variant: maps of the two images / the state volume
+    RfaTensorMap tm_blk_state[RFA_N_SHAPES]{};      // per tile shape
+    // Residual-prefetch variant of the blocked kernel (rfa_kernels.cu: RPF): chosen from the share of warp-planes that took
+    // the compensated path, which the kernels count in counters[5]; the count is read back without ever waiting for the
+    // stream (an 8-byte copy into pinned memory + an event that later launches poll)
+    int res_prefetch_mode = RFA_RES_PREFETCH_AUTO;
+    int res_prefetch_on = 0;
+    unsigned long long *hot_host = nullptr;   // pinned
+    cudaEvent_t hot_evt = nullptr;
+    bool hot_pending = false;
+    unsigned long long hot_seen = 0;          // counter value at the last completed sample
+    double planes_issued = 0, planes_at_sample = 0, planes_seen = 0;   // warp-planes launched: now / at the pending sample / at the last completed one
+    double hot_fraction = 0;                  // last completed sample
+    int launches_since_sample = 0;
+    int staging = RFA_STAGING_AUTO;      // rfa_configure_staging
+    int force_shape = -1;                // rfa_configure_tile: -1 = the planner chooses
     int device = 0;                      // the CUDA device the simulation lives on (current device at rfa_create)
     int held_copy_auto = 0;              // what rfa_create chose for the held-copy variant (RFA_HELD_COPY_AUTO)
 };
@@ -213,17 +229,23 @@ static void build_table(const rfa_sim *s, double q_power, RfaTableHost &out)
 // ------------------------------------------------------------------------------------------------
 // plan of the blocked kernel (host only)
 // ------------------------------------------------------------------------------------------------
-static RfaTbPlan plan_shape(int nx, int ny, int nz, int batch, int S, int shape, int resident_ctas, double &cost_out)
+static RfaTbPlan plan_shape(int nx, int ny, int nz, int batch, int S, int shape, int resident_ctas, int tma, double &cost_out)
 {
     RfaTbPlan p{};
     p.fused = S;
     p.shape = shape;
+    p.tma = tma;
     cost_out = 1e300;
     if (resident_ctas < 1) return p;
-    const int BX = 4 * RFA_TB_SHAPE[shape][S].tx, BY = RFA_TB_SHAPE[shape][S].ry * RFA_TB_SHAPE[shape][S].ty;
+    const int RY = RFA_TB_SHAPE[shape][S].ry;
+    const int BX = 4 * RFA_TB_SHAPE[shape][S].tx, BY = RY * RFA_TB_SHAPE[shape][S].ty;
     if (BY <= 2 * S) return p;
+    // TMA-staged variant: Eq. 12 kernels with 2 or 3 fused steps, state rows of a multiple of 16 bytes, whole thread rows
+    if (tma && (S < 2 || S > 3 || (nx % 16) != 0 || (ny % RY) != 0)) return p;
+    // its first tile starts SR = S rounded up to a multiple of RY rows above the grid (rfa_kernels.cu), SR - S more than needed
+    const int lead = tma ? (S + RY - 1) / RY * RY - S : 0;
     p.tiles_x = nx <= BX ? 1 : (nx - 8 + (BX - 8) - 1) / (BX - 8);
-    p.tiles_y = (ny + (BY - 2 * S) - 1) / (BY - 2 * S);
+    p.tiles_y = (ny + lead + (BY - 2 * S) - 1) / (BY - 2 * S);
     const long long per_z = (long long)p.tiles_x * p.tiles_y * batch;
     // choose the number of z chunks: minimise rounds * (planes streamed per item + fixed cost)
     double best = 1e300;
@@ -248,10 +270,11 @@ static RfaTbPlan plan_shape(int nx, int ny, int nz, int batch, int S, int shape,
     return p;
 }
 
-RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const int resident_ctas[RFA_N_SHAPES])
+RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const int resident_ctas[RFA_N_SHAPES], int tma)
 {
     RfaTbPlan best{};
     best.fused = fused;
+    best.tma = tma;
     const int S = fused;
     if (S < 1 || S > 4 || nx < 4 || (nx % 4) != 0 || ny < S || nz < S || batch < 1 || !resident_ctas) return best;
     // the kernel addresses one scenario with 32-bit float4 offsets; larger volumes take the plain kernel
@@ -259,7 +282,7 @@ RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const i
     double best_cost = 1e300;
     for (int shape = 0; shape < RFA_N_SHAPES; ++shape) {
         double cost;
-        RfaTbPlan p = plan_shape(nx, ny, nz, batch, S, shape, resident_ctas[shape], cost);
+        RfaTbPlan p = plan_shape(nx, ny, nz, batch, S, shape, resident_ctas[shape], tma, cost);
         // every CTA has 256 threads and 8 voxels per thread and plane, so plane iterations compare directly;
         // the wide shape must win by 5 % (its y halo costs more redundant rows per useful one)
         if (p.ok && cost < best_cost * (shape == 0 ? 1.0 : 0.95)) {
@@ -305,11 +328,12 @@ RfaTbPlan rfa_plan_stream(int nx, int ny, int nz, int batch, int resident_ctas)
 }
 
 // exported for the CPU unit tests of the planner (no GPU needed)
-extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resident_ctas, int out[9])
+extern "C" int rfa_plan_query(const int dims[3], int batch, int fused, int resident_ctas, int staging, int out[9])
 {
     if (!dims || !out) return RFA_E_INVALID;
+    if (staging != RFA_STAGING_CP_ASYNC && staging != RFA_STAGING_TMA) return RFA_E_INVALID;
     const int res[RFA_N_SHAPES] = {resident_ctas, resident_ctas};
-    RfaTbPlan p = rfa_plan_blocked(dims[0], dims[1], dims[2], batch, fused, res);
+    RfaTbPlan p = rfa_plan_blocked(dims[0], dims[1], dims[2], batch, fused, res, staging == RFA_STAGING_TMA ? 1 : 0);
     out[0] = p.ok;
     out[1] = p.tiles_x;
     out[2] = p.tiles_y;
@@ -367,10 +391,31 @@ static void make_plans(rfa_sim *s)
                    rfa_stream_make_maps(s->g, s->theta[1], nullptr, &s->tm_theta[1], nullptr);
     s->stream_plan = s->stream_ok ? rfa_plan_stream(s->g.nx, s->g.ny, s->g.nz, s->g.batch, rfa_stream_resident_ctas()) : RfaTbPlan{};
     if (!s->stream_plan.ok) s->stream_ok = false;
+    // tensor maps of the blocked kernel's TMA variant: box = the tile of each shape (the same for 2 and 3 fused steps)
+    bool blk_maps[RFA_N_SHAPES];
+    for (int sh = 0; sh < RFA_N_SHAPES; ++sh) {
+        int bx = 0, by = 0, bx3 = 0, by3 = 0;
+        rfa_blocked_tile(2, sh, &bx, &by);
+        rfa_blocked_tile(3, sh, &bx3, &by3);
+        blk_maps[sh] = bx == bx3 && by == by3 && rfa_make_tile_map(s->g, s->theta[0], 4, bx, by, &s->tm_blk_theta[0][sh]) &&
+                       rfa_make_tile_map(s->g, s->theta[1], 4, bx, by, &s->tm_blk_theta[1][sh]) &&
+                       rfa_make_tile_map(s->g, s->state, 1, bx + 16, by, &s->tm_blk_state[sh]);
+    }
     for (int f = 1; f <= 4; ++f) {
         for (int m = 0; m < 2; ++m) {
-            for (int sh = 0; sh < RFA_N_SHAPES; ++sh) s->resident[m][f][sh] = rfa_blocked_resident_ctas(f, sh, m);
-            s->plans_by_mode[m][f] = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, s->resident[m][f]);
+            int res_tma[RFA_N_SHAPES];
+            for (int sh = 0; sh < RFA_N_SHAPES; ++sh) {
+                const bool want = s->force_shape < 0 || s->force_shape == sh;
+                s->resident[m][f][sh] = want ? rfa_blocked_resident_ctas(f, sh, m, 0) : 0;
+                res_tma[sh] = (want && m == 0 && blk_maps[sh] && s->staging != RFA_STAGING_CP_ASYNC) ? rfa_blocked_resident_ctas(f, sh, m, 1) : 0;
+            }
+            // AUTO: the TMA-staged variant where it measured faster on the B200 -- the 128 x 16 tile (C5: 684 -> 704 GVox/s);
+            // with the 64 x 32 tile the elected thread's issue sequence sits on the critical path of the per-plane barrier
+            // and the per-thread cp.async variant wins (C4: 783 vs 707), profiles/r2_blocked_tma_vs_cpasync.md
+            const RfaTbPlan pc = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, s->resident[m][f], 0);
+            const RfaTbPlan pt = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, res_tma, 1);
+            const bool take_tma = pt.ok && (s->staging == RFA_STAGING_TMA || !pc.ok || (pt.shape == 1 && pc.shape == 1));
+            s->plans_by_mode[m][f] = take_tma ? pt : pc;
         }
     }
 }
@@ -517,8 +562,12 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     int rc = RFA_OK;
     do {
         // labels -> device (staged through scratch), then label -> initial temperature image
-        e = cudaMemsetAsync(s->counters, 0, 256, s->stream);   // necrotic-voxel counts [0..1], dynamic work counter [4]
+        e = cudaMemsetAsync(s->counters, 0, 256, s->stream);   // necrotic-voxel counts [0..1], dynamic work counter [4], hot warp-planes [5]
         if (e != cudaSuccess) { rc = cuda_fail(e, "counter reset"); break; }
+        // feedback channel of the residual-prefetch choice; without it the variant simply stays off
+        if (cudaHostAlloc((void **)&s->hot_host, 64, cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); s->hot_host = nullptr; }
+        else *s->hot_host = 0;
+        if (cudaEventCreateWithFlags(&s->hot_evt, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); s->hot_evt = nullptr; }
         e = cudaMemcpyAsync(s->scratch, labels, nvox, cudaMemcpyHostToDevice, s->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "label upload"); break; }
         float theta0[RFA_NLABEL], kl[RFA_NLABEL], kap[RFA_NLABEL * RFA_NLABEL];
@@ -565,6 +614,8 @@ extern "C" void rfa_destroy(rfa_sim *s)
         if (s->probes) cudaFree(s->probes);
         if (s->record) cudaFree(s->record);
         if (s->stage) cudaFree(s->stage);
+        if (s->hot_host) cudaFreeHost(s->hot_host);
+        if (s->hot_evt) cudaEventDestroy(s->hot_evt);
     }
     delete s;
 }
@@ -686,6 +737,57 @@ extern "C" int rfa_configure_held_copy(rfa_sim *s, int mode)
     return RFA_OK;
 }
 
+extern "C" int rfa_configure_staging(rfa_sim *s, int mode)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (mode != RFA_STAGING_AUTO && mode != RFA_STAGING_CP_ASYNC && mode != RFA_STAGING_TMA)
+        return fail(RFA_E_INVALID, "bad staging mode %d", mode);
+    DeviceGuard dg(s);
+    const int old = s->staging;
+    s->staging = mode;
+    make_plans(s);
+    if (mode == RFA_STAGING_TMA && !(s->plans_by_mode[0][2].tma || s->plans_by_mode[0][3].tma)) {
+        s->staging = old;
+        make_plans(s);
+        return fail(RFA_E_INVALID, "no TMA-staged variant for this grid (needs nx %% 16 == 0, ny even; grid %dx%dx%d)", s->g.nx, s->g.ny, s->g.nz);
+    }
+    if (s->kernel == RFA_KERNEL_BLOCKED && !s->plans()[s->fused].ok) s->kernel = RFA_KERNEL_AUTO;
+    return RFA_OK;
+}
+
+extern "C" int rfa_configure_residual_prefetch(rfa_sim *s, int mode)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (mode != RFA_RES_PREFETCH_AUTO && mode != RFA_RES_PREFETCH_OFF && mode != RFA_RES_PREFETCH_ON)
+        return fail(RFA_E_INVALID, "bad residual-prefetch mode %d", mode);
+    s->res_prefetch_mode = mode;
+    return RFA_OK;
+}
+
+extern "C" int rfa_query_hot_fraction(rfa_sim *s, double *fraction, int *prefetch_on)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (fraction) *fraction = s->hot_fraction;
+    if (prefetch_on) *prefetch_on = s->res_prefetch_mode == RFA_RES_PREFETCH_AUTO ? s->res_prefetch_on : s->res_prefetch_mode;
+    return RFA_OK;
+}
+
+extern "C" int rfa_configure_tile(rfa_sim *s, int shape)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    if (shape < -1 || shape >= RFA_N_SHAPES) return fail(RFA_E_INVALID, "tile shape must be -1 (planner's choice), 0 (64 x 32) or 1 (128 x 16)");
+    DeviceGuard dg(s);
+    const int old = s->force_shape;
+    s->force_shape = shape;
+    make_plans(s);
+    if (s->kernel == RFA_KERNEL_BLOCKED && !s->plans()[s->fused].ok) {
+        s->force_shape = old;
+        make_plans(s);
+        return fail(RFA_E_INVALID, "tile shape %d cannot run the configured %d fused steps on this grid", shape, s->fused);
+    }
+    return RFA_OK;
+}
+
 extern "C" int rfa_set_conduction(rfa_sim *s, int mode)
 {
     if (!s) return fail(RFA_E_INVALID, "null simulation handle");
@@ -717,6 +819,56 @@ extern "C" int rfa_query(rfa_sim *s, int *kernel, int *fused_steps, int64_t *ker
     return RFA_OK;
 }
 
+// Feedback for the residual-prefetch variant: every RFA_HOT_SAMPLE_EVERY launches the hot warp-plane counter is copied to
+// pinned memory behind the launches issued so far; a later call finds the copy complete (cudaEventQuery, never a wait) and
+// switches the variant on above RFA_HOT_ON of the warp-planes, off below RFA_HOT_OFF.  Both variants give bit-identical
+// fields, so the switch changes speed only.  Measured on the B200: the variant costs 2.4 % where next to nothing is hot
+// (C4: 0.17 % of the warp-planes, 770 -> 752 GVox/s), is neutral at 1.1 % (C5), gains 8 % at 2.2 % (C3 after 3000
+// steps, 452 -> 487) and 11 % at 84 % (C4F, 290 -> 322): break-even near 0.5 %.
+#define RFA_HOT_SAMPLE_EVERY 32
+#define RFA_HOT_ON 0.004
+#define RFA_HOT_OFF 0.0025
+static void sample_hot_fraction(rfa_sim *s, const RfaTbPlan &pl)
+{
+    s->planes_issued += (double)pl.n_items * (pl.zchunk + 2 * pl.fused) * 8.0;       // 8 warps per CTA
+    if (!s->hot_host || !s->hot_evt) return;
+    if (s->hot_pending) {
+        ++s->launches_since_sample;
+        if (s->res_prefetch_mode == RFA_RES_PREFETCH_AUTO && s->launches_since_sample >= 2 * RFA_HOT_SAMPLE_EVERY) {
+            // The host has run RFA_HOT_SAMPLE_EVERY launches past the sample and the device has not reached it yet: wait for
+            // it here.  The device still has those launches queued, so it never idles; the host just stops running further
+            // ahead of it than the feedback can follow (a single rfa_step(12000) would otherwise issue every launch with
+            // the choice made before the first one ran).
+            if (cudaEventSynchronize(s->hot_evt) != cudaSuccess) { cudaGetLastError(); return; }
+        } else if (cudaEventQuery(s->hot_evt) != cudaSuccess) {
+            cudaGetLastError();                              // not ready yet: ask again at the next launch
+            return;
+        }
+        const unsigned long long now = *s->hot_host;
+        const double planes = s->planes_at_sample - s->planes_seen;
+        if (planes > 0) {
+            s->hot_fraction = (double)(now - s->hot_seen) / planes;
+            if (s->hot_fraction >= RFA_HOT_ON) s->res_prefetch_on = 1;
+            else if (s->hot_fraction < RFA_HOT_OFF) s->res_prefetch_on = 0;
+        }
+        s->hot_seen = now;
+        s->planes_seen = s->planes_at_sample;
+        s->hot_pending = false;
+        s->launches_since_sample = 0;
+        return;
+    }
+    if (++s->launches_since_sample >= RFA_HOT_SAMPLE_EVERY) {
+        if (cudaMemcpyAsync(s->hot_host, s->counters + 5, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s->stream) == cudaSuccess &&
+            cudaEventRecord(s->hot_evt, s->stream) == cudaSuccess) {
+            s->hot_pending = true;
+            s->launches_since_sample = RFA_HOT_SAMPLE_EVERY;
+            s->planes_at_sample = s->planes_issued;
+        } else {
+            cudaGetLastError();
+        }
+    }
+}
+
 // n time steps on the stream: launches of up to `fused` steps each, buffers swapped per launch (Alg. 2)
 static int advance(rfa_sim *s, int n)
 {
@@ -735,8 +887,13 @@ static int advance(rfa_sim *s, int n)
                                   s->counters + 4, s->stream_draws, s->stream);
             s->stream_draws += (unsigned long long)s->stream_plan.n_items;   // every launch draws exactly n_items times
         }
-        else if (k == RFA_KERNEL_BLOCKED)
-            e = rfa_launch_blocked(s->g, s->plans()[did], tin, tout, rin, rout, s->state, s->tables, kap, s->stream);
+        else if (k == RFA_KERNEL_BLOCKED) {
+            const RfaTbPlan &pl = s->plans()[did];
+            const int rpf = s->res_prefetch_mode == RFA_RES_PREFETCH_AUTO ? s->res_prefetch_on : s->res_prefetch_mode;
+            e = rfa_launch_blocked(s->g, pl, tin, tout, rin, rout, s->state, s->tables, kap, &s->tm_blk_theta[s->cur][pl.shape],
+                                   &s->tm_blk_state[pl.shape], rpf && rfa_blocked_has_prefetch(did, pl.tma), s->counters + 5, s->stream);
+            if (e == cudaSuccess) sample_hot_fraction(s, pl);
+        }
         else {
             did = 1;
             e = rfa_launch_plain(s->g, tin, tout, rin, rout, s->state, s->tables, kap, s->stream);
@@ -749,7 +906,7 @@ static int advance(rfa_sim *s, int n)
     return RFA_OK;
 }
 
-extern "C" int rfa_query_variant(rfa_sim *s, int out[6])
+extern "C" int rfa_query_variant(rfa_sim *s, int out[8])
 {
     if (!s || !out) return fail(RFA_E_INVALID, "null argument");
     const int k = kernel_for(s, s->fused);
@@ -761,6 +918,9 @@ extern "C" int rfa_query_variant(rfa_sim *s, int out[6])
     out[3] = blocked ? p.grid : (stream ? s->stream_plan.grid : 0);
     out[4] = (blocked || stream) ? s->g.held_copy : 0;
     out[5] = s->conduction;
+    out[6] = stream ? RFA_STAGING_TMA : (blocked && p.tma ? RFA_STAGING_TMA : RFA_STAGING_CP_ASYNC);
+    const int rpf = s->res_prefetch_mode == RFA_RES_PREFETCH_AUTO ? s->res_prefetch_on : s->res_prefetch_mode;
+    out[7] = (blocked && rpf && rfa_blocked_has_prefetch(s->fused, p.tma)) ? 1 : 0;
     return RFA_OK;
 }
 

@@ -25,6 +25,7 @@ struct RfaTbPlan {
     int n_items;               // batch * nzc * tiles_y * tiles_x
     int grid;                  // CTAs launched (persistent, static round-robin over items)
     int ok;                    // 0: this grid cannot use the blocked kernel
+    int tma;                   // 1: the variant whose level-0 planes are staged by the Tensor Memory Accelerator
 };
 
 // tile shape of the blocked kernel per number of fused steps S (index 1..4): TX x TY threads, each owning
@@ -73,7 +74,8 @@ constexpr RfaTbShape RFA_TB_SHAPE[RFA_N_SHAPES][5] = {{{0, 0, 0, 0},
 
 // host-only planning (no CUDA calls): implemented in rfa_api.cpp, unit-tested on CPU
 // resident_ctas: co-resident CTAs per shape (0 = this shape cannot run)
-RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const int resident_ctas[RFA_N_SHAPES]);
+// tma = 1: plan for the TMA-staged variant (tiles start RY-aligned above the grid: one more halo row at S = 3)
+RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const int resident_ctas[RFA_N_SHAPES], int tma = 0);
 
 // launchers (rfa_kernels.cu).  All asynchronous on `st`; return cudaGetLastError().
 cudaError_t rfa_launch_table(const RfaTableHost &tbl, float *dst, cudaStream_t st);
@@ -107,9 +109,15 @@ cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *stat
 // kap: null = Eq. 12 as printed; else device table [16][16] of Kf/K_c - 1 (conservative conduction, R-28)
 cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, const void *rin, void *rout,
                              uint8_t *state, const float *tables, const float *kap, cudaStream_t st);
+struct RfaTensorMap;
+// map_theta_in / map_state: tensor maps (box = the plan's tile) of the input image and the state volume; used when plan.tma
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
                                const void *rin, void *rout, uint8_t *state, const float *tables, const float *kap,
-                               cudaStream_t st);
+                               const RfaTensorMap *map_theta_in, const RfaTensorMap *map_state, int res_prefetch,
+                               unsigned long long *hot_ctr /*device: += hot warp-planes*/, cudaStream_t st);
+// 1: a kernel variant that prefetches the level-0 residual rows of hot planes exists for this number of fused steps / staging
+int rfa_blocked_has_prefetch(int fused, int tma);
+void rfa_blocked_tile(int fused, int shape, int *bx, int *by);
 // ---- one-step kernel staged by the Tensor Memory Accelerator (rfa_stream.cu) ----------------------------------------
 // tile of one CTA: RFA_STREAM_BX x RFA_STREAM_BY voxels (8 warps x RFA_STREAM_RY rows, one float4 column per lane), a ring of
 // RFA_STREAM_D shared-memory slots per CTA (D - 2 planes in flight).  Measured on the B200 (C4, us per step): 2 rows per
@@ -134,6 +142,8 @@ struct alignas(64) RfaTensorMap {
 };
 // tensor maps of one fp32 image / of the packed state volume, both seen as (nx, ny, nz * batch); either output may be null.
 // false: no TMA path for this grid (nx % 16 != 0) or no driver entry point
+// general form: box_x x box_y x 1 elements of 4 (fp32 image) or 1 (state volume) bytes
+bool rfa_make_tile_map(const RfaGrid &g, const void *base, int elem_bytes, int box_x, int box_y, RfaTensorMap *out);
 bool rfa_stream_make_maps(const RfaGrid &g, const float *theta, const uint8_t *state, RfaTensorMap *map_theta, RfaTensorMap *map_state);
 int rfa_stream_resident_ctas();
 // plan fields used: tiles_x, tiles_y, nzc, zchunk, n_items, grid
@@ -145,4 +155,4 @@ cudaError_t rfa_launch_stream(const RfaGrid &g, const RfaTbPlan &plan, const Rfa
 
 // resident CTAs of the blocked kernel on the current device for `fused` steps (occupancy * SM count);
 // cons = 1: the conservative-conduction variant
-int rfa_blocked_resident_ctas(int fused, int shape, int cons);
+int rfa_blocked_resident_ctas(int fused, int shape, int cons, int tma = 0);

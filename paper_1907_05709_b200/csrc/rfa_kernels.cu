@@ -26,6 +26,11 @@ __device__ __forceinline__ void cp_async4(void *smem_dst, const void *gsrc)
     unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(d), "l"(gsrc) : "memory");
 }
+__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
+{
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gsrc) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait()
@@ -237,7 +242,8 @@ __global__ void rfa_plain_kernel(RfaGrid g, const float *__restrict__ tin, float
 // (ghost -1 = row 0, -2 = row 1, ...), which reproduces the zero-flux replicate rule exactly through
 // all S levels because the update is symmetric in (ym,yp) and (zm,zp) bit for bit.  At the outer x
 // faces the replicate rule is applied directly (a select on the two edge lanes).
-struct RfaTbParams {
+struct alignas(64) RfaTbParams {
+    RfaTensorMap tm_theta, tm_state;  // TMA variant: tensor maps of the input image and of the state volume (box = the tile)
     const float *tin;
     float *tout;
     const __half *rin;
@@ -250,11 +256,13 @@ struct RfaTbParams {
     float wx, wy, wz, thr;
     int tiles_x, tiles_y, nzc, zchunk, n_items;
     int held_copy;                    // kernel variant: warps of held voxels only copy their rows (HELDCOPY)
+    int res_prefetch;                 // kernel variant: level-0 residual rows of hot planes are prefetched (RPF)
+    unsigned long long *hot_ctr;      // += warp-planes that took the compensated path at level 0 (never reset)
 };
 
 constexpr int rfa_pow2_at_least(int n) { return n <= 1 ? 1 : 2 * rfa_pow2_at_least((n + 1) / 2); }
 
-template <int S, int TX, int TY, int RY, bool CONS = false>
+template <int S, int TX, int TY, int RY, bool CONS = false, bool TMA = false, bool RPF = false>
 struct TbCfg {
     static constexpr int NT = TX * TY;
     static constexpr int BX = 4 * TX;
@@ -263,23 +271,38 @@ struct TbCfg {
 #define RFA_S1_PD 1
 #endif
     // prefetch distance (planes in flight): the one-step kernel is bound by memory latency, not by issue slots
-    static constexpr int PD = S == 1 ? RFA_S1_PD : 1;
-    static constexpr int DT = rfa_pow2_at_least(PD + 1);          // temperature ring depth
+    // (TMA variant: two planes in flight, a ring of three slots indexed by the iteration number mod 3 = the unrolled body)
+    static constexpr int PD = TMA ? 2 : (S == 1 ? RFA_S1_PD : 1);
+    static constexpr int DT = TMA ? 3 : rfa_pow2_at_least(PD + 1);          // temperature ring depth
     // state ring depth: level k reads plane i-k-1; the conservative mode also reads the planes i-k and i-k-2 and
     // the rows of the neighbouring threads (one extra slot keeps a thread one barrier ahead off them)
     static constexpr int DS = rfa_pow2_at_least(CONS ? PD + S + 3 : PD + S + 1);
     static constexpr int NR = S > 1 ? S - 1 : 1;                  // inter-level residual buffers
     static constexpr size_t RING_T = (size_t)DT * RY * NT * 16;
     static constexpr size_t EXCH = (size_t)S * 2 * 2 * NT * 16;
-    static constexpr size_t RING_S = (size_t)DS * RY * NT * 4;
+    // TMA variant: the copy engine wants the box of the byte volume to start on a 16-byte boundary in x (a box at x = 56
+    // faults), while tiles start every BX - 8 voxels: the state box starts at the boundary at or below the tile and is 16 bytes wider
+    static constexpr int SROW = TMA ? TX + 4 : TX;                // state words per tile row in shared memory
+    static constexpr size_t RING_S = (size_t)DS * RY * TY * SROW * 4;
     static constexpr size_t RSM = S > 1 ? (size_t)NR * 2 * RY * NT * 8 : 0;
     static constexpr size_t TAB = 3 * RFA_TABLE_N * 4;
     static constexpr size_t KAP = CONS ? RFA_NLABEL * RFA_NLABEL * 4 : 0;
-    static constexpr size_t SMEM = RING_T + EXCH + RING_S + RSM + TAB + KAP;
+    static constexpr size_t BARS = TMA ? DT * 8 : 0;              // one mbarrier per temperature slot
+    // level-0 residuals of hot rows are prefetched (cp.async, 8 bytes per row) one iteration ahead into a two-slot ring
+    // instead of being loaded where they are used (the 3-step TMA variants have no shared memory left for it)
+    // -- a kernel variant of its own (RPF): +12..14 % where a good part of the volume is hot (C3, C4F), -3 % where next to
+    // nothing is (C4: the added code is not free in a kernel that already stalls on instruction fetch); the library picks
+    // the variant from the share of hot warp-planes the kernels themselves count (rfa_api.cpp: advance)
+    static constexpr bool RESPF = RPF && (!TMA || S == 2);
+    static constexpr size_t RESQ = RESPF ? (size_t)2 * RY * NT * 8 : 0;
+    static constexpr size_t SMEM = RING_T + EXCH + RING_S + RSM + TAB + KAP + RESQ + BARS;
+    static constexpr int SR = ((S + RY - 1) / RY) * RY;           // TMA variant: halo rows above the first tile (a multiple of RY)
+    static_assert(!TMA || (!CONS && S >= 2 && RY == 2), "TMA variant: Eq. 12 mode, S >= 2, two rows per thread");
 };
 
 #define RFA_MAX_DEVICES 64
 #include "rfa_packed.cuh"
+#include "rfa_tma.cuh"
 
 // Conservative conduction, one row of four voxels (rfa_device.cuh: rfa_face_correction; R-28): g of
 // every voxel whose interface bit is set gets the face correction added.  w = the row's state word, w?? = the
@@ -315,24 +338,38 @@ struct IC {
     static constexpr int value = I;
 };
 
-template <int S, int TX, int TY, int RY, int MINB, bool CONS, bool HELDCOPY>
-__global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbParams P)
+template <int S, int TX, int TY, int RY, int MINB, bool CONS, bool HELDCOPY, bool TMA, bool RPF>
+__global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_constant__ RfaTbParams P)
 {
-    using C = TbCfg<S, TX, TY, RY, CONS>;
+    using C = TbCfg<S, TX, TY, RY, CONS, TMA, RPF>;
     constexpr int NT = C::NT, BX = C::BX, BY = C::BY, PD = C::PD, DT = C::DT, DS = C::DS;
     static_assert(RY == 4 || RY == 2, "state words of a thread are read as one vector");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4 *ringT = reinterpret_cast<float4 *>(smem_raw);                                          // [DT][RY][NT]
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4 *ringT = reinterpret_cast<float4 *>(smem_raw);                                          // [DT][RY][NT]; TMA: [DT][BY][TX]
     float4 *exch = reinterpret_cast<float4 *>(smem_raw + C::RING_T);                               // [S][2 parity][2 top/bot][NT]
-    uint32_t *ringS = reinterpret_cast<uint32_t *>(smem_raw + C::RING_T + C::EXCH);                // [DS][NT][RY]
+    uint32_t *ringS = reinterpret_cast<uint32_t *>(smem_raw + C::RING_T + C::EXCH);                // [DS][NT][RY]; TMA: [DS][BY][TX]
     uint2 *rsm = reinterpret_cast<uint2 *>(smem_raw + C::RING_T + C::EXCH + C::RING_S);            // [NR][2 parity][RY][NT]
     float *tab = reinterpret_cast<float *>(smem_raw + C::RING_T + C::EXCH + C::RING_S + C::RSM);   // [3][128]
     float *kap = tab + 3 * RFA_TABLE_N;                                                            // [16][16] (CONS)
+    uint2 *resq = reinterpret_cast<uint2 *>(smem_raw + C::SMEM - C::BARS - C::RESQ);               // [2][RY][NT] (RESPF)
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + C::SMEM - C::BARS);                   // [DT] plane landed (TMA)
 
     const int tid = threadIdx.x;
     const int tx = tid % TX, ty = tid / TX;
     const int up_tid = (ty > 0 ? ty - 1 : ty) * TX + tx;
     const int dn_tid = (ty < TY - 1 ? ty + 1 : ty) * TX + tx;
+    // shared-memory words of this thread's rows inside one ring slot (temperature: float4 units, state: 32-bit words)
+    auto t_idx = [&](const int slot, const int r) { return TMA ? (slot * BY + ty * RY + r) * TX + tx : (slot * RY + r) * NT + tid; };
+    int s_off = tx;                                          // TMA: word of this thread's column inside a state row (set per item)
+    auto s_idx = [&](const int slot, const int r) { return TMA ? (slot * BY + ty * RY + r) * C::SROW + s_off : (slot * NT + tid) * RY + r; };
+    if constexpr (TMA) {
+        if (tid == 0) {
+#pragma unroll
+            for (int s = 0; s < DT; ++s) mbar_init(&full[s], 1);
+            mbar_fence_init();
+        }
+    }
+    unsigned phases = 0;                                     // TMA: bit s = parity of the next completion of full[s]
 
     for (int e = tid; e < S * 2 * 2 * NT; e += NT) exch[e] = make_float4(0.f, 0.f, 0.f, 0.f);
     if constexpr (CONS)
@@ -354,7 +391,10 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
         const int zc = t % P.nzc;
         const int b = t / P.nzc;
         const int X0 = txi * (BX - 8);
-        const int Y0 = -S + tyi * (BY - 2 * S);
+        // TMA variant: the tile starts a multiple of RY rows above the grid, so that row 0 is some thread's first row and
+        // (ny being a multiple of RY) row ny-1 some thread's last one: the zero-flux rule at the outer y faces is then a
+        // matter of which exchange entry a thread reads (its own row instead of the neighbour's), not of mirrored loads
+        const int Y0 = (TMA ? -C::SR : -S) + tyi * (BY - 2 * S);
         const int z0 = zc * P.zchunk;
         const int z1 = min(z0 + P.zchunk, P.nz);
 
@@ -372,6 +412,14 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
             if (ly >= S && ly < BY - S && gy >= 0 && gy < P.ny && col_ok) row_ok |= 1u << r;
             row_src[r] = (unsigned)(rfa_reflect(gy, P.ny) * P.nx4 + gx4c);
             row_dst[r] = (unsigned)(min(max(gy, 0), P.ny - 1) * P.nx4 + gx4c);
+        }
+        // exchange entries of the rows above / below this thread's rows: [0] = a thread's first row, [1] = its last row
+        int up_idx = NT + up_tid, dn_idx = dn_tid;
+        if constexpr (TMA) {
+            s_off = tx + (X0 & 15) / 4;
+            const int gyf = Y0 + ty * RY;
+            if (gyf == 0) up_idx = tid;                      // outer faces: the voxel itself (R-7)
+            if (gyf + RY == P.ny) dn_idx = NT + tid;
         }
         const size_t base4 = (size_t)b * P.nz * plane4;
         const float4 *tin4 = reinterpret_cast<const float4 *>(P.tin) + base4;
@@ -392,6 +440,8 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
         float4 q[S][3][RY];
         unsigned nbq[S][3];
         bool hotq[S][3], rvq[S][3];
+        unsigned hot_planes = 0;                         // warp-planes of this item on the compensated path at level 0
+        bool coldq0[3] = {true, true, true};             // level 0: no thread of the warp has a hot voxel in the plane (the vote, taken on arrival)
 #pragma unroll
         for (int k = 0; k < S; ++k)
 #pragma unroll
@@ -413,10 +463,25 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 cp_async4(&ringS[(sS * NT + tid) * RY + r], st4 + (pl + row_src[r]));
             }
         };
+        // TMA variant: ONE thread hands plane j of the item (tile box at (X0, Y0), z mirrored at the outer faces) to the copy
+        // engine; parts of the box outside the grid arrive as zeros and are never used by a voxel that is stored
+        auto issue_tma = [&](const int j, const int sT) {
+            const int pz = b * P.nz + rfa_reflect(z0 - S + j, P.nz);
+            mbar_expect_tx(&full[sT], (uint32_t)(BX * BY * 4 + C::SROW * 4 * BY));
+            tma_load_3d(ringT + sT * BY * TX, &P.tm_theta, &full[sT], X0, Y0, pz);
+            tma_load_3d(ringS + (j & (DS - 1)) * BY * C::SROW, &P.tm_state, &full[sT], X0 & ~15, Y0, pz);
+        };
+        if constexpr (TMA) {
+            if (tid == 0) {
+                issue_tma(0, 0);
+                issue_tma(1, 1);                             // niter >= 2 S + 1 > 2
+            }
+        } else {
 #pragma unroll
-        for (int j = 0; j < PD; ++j) {
-            if (j < niter) issue(j);
-            cp_async_commit();
+            for (int j = 0; j < PD; ++j) {
+                if (j < niter) issue(j);
+                cp_async_commit();
+            }
         }
 
         // one plane iteration; PH = i mod 3 selects the register slots at compile time
@@ -424,19 +489,43 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
             constexpr int PH = decltype(ph)::value;
             constexpr int CE = (PH + 2) % 3;               // centre plane slot
             constexpr int MI = (PH + 1) % 3;               // previous plane slot
-            if (i + PD < niter) issue(i + PD);
-            cp_async_commit();
-            cp_async_wait<PD>();
+            if constexpr (TMA) {
+                mbar_wait(&full[PH], (phases >> PH) & 1u);
+                phases ^= 1u << PH;
+                if constexpr (C::RESPF) cp_async_wait<0>();          // residual rows of the centre plane (issued one iteration ago)
+            } else {
+                if (i + PD < niter) issue(i + PD);
+                cp_async_commit();
+                // all but the youngest group: this iteration's plane and (RESPF) last iteration's residual rows have landed
+                static_assert(PD == 1, "the residual prefetch group sits between two plane groups");
+                cp_async_wait<PD>();
+            }
             {
-                const int sT = i & (DT - 1);
+                const int sT = TMA ? PH : (i & (DT - 1));
                 float m = 0.f;
 #pragma unroll
                 for (int r = 0; r < RY; ++r) {
-                    q[0][PH][r] = ringT[(sT * RY + r) * NT + tid];
+                    q[0][PH][r] = ringT[t_idx(sT, r)];
                     m = max_abs4(q[0][PH][r], m);
                 }
                 nbq[0][PH] = 0;
                 hotq[0][PH] = m >= RFA_COMP_MIN;
+                // the level-0 vote of the NEXT iteration, taken now: a warp-uniform flag, so the prefetch below costs a cold warp
+                // one uniform branch
+                if constexpr (C::RESPF) {
+                    coldq0[PH] = __all_sync(0xffffffffu, !hotq[0][PH]);
+                    // this plane is the centre plane of the next iteration: fetch the residuals of its hot rows now (cp.async,
+                    // 8 bytes per row), so that the hot path finds them in shared memory instead of waiting for L2 in the
+                    // middle of level 0 while the warp's whole CTA waits at the barrier
+                    if (!coldq0[PH] && hotq[0][PH]) {
+                        const unsigned pla = (unsigned)rfa_reflect(z0 - S + i, P.nz) * plane4;
+#pragma unroll
+                        for (int r = 0; r < RY; ++r) cp_async8(&resq[((i & 1) * RY + r) * NT + tid], rin2 + (pla + row_src[r]));
+                        // a group of its own, committed by the hot threads only: cp.async groups are per thread, and for a
+                        // thread that has one it sits between two plane groups, so the wait above covers it either way
+                        cp_async_commit();
+                    }
+                }
             }
             // state words of the S centre planes and the two warp votes per level that pick the code path:
             // thread-private data, so all of it is issued before the barrier and overlaps the wait
@@ -445,7 +534,10 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
 #pragma unroll
             for (int k = 0; k < S; ++k) {
                 const int sS = (i - (k + 1)) & (DS - 1);
-                if constexpr (RY == 4) {
+                if constexpr (TMA) {
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) sw[k][r] = ringS[s_idx(sS, r)];
+                } else if constexpr (RY == 4) {
                     const uint4 v = *reinterpret_cast<const uint4 *>(&ringS[(sS * NT + tid) * RY]);
                     sw[k][0] = v.x; sw[k][1] = v.y; sw[k][2] = v.z; sw[k][3] = v.w;
                 } else {
@@ -464,9 +556,13 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                     one = one && !ifc[k];
                 }
                 uni[k] = __all_sync(0xffffffffu, one);
-                cold[k] = __all_sync(0xffffffffu, !hotq[k][CE]);                  // all residuals are zero
+                cold[k] = (C::RESPF && k == 0) ? coldq0[CE] : __all_sync(0xffffffffu, !hotq[k][CE]);   // all residuals are zero
             }
             __syncthreads();                               // exchange rows of iteration i-1 are visible
+            if constexpr (TMA) {
+                // every thread has taken plane i-1 out of its slot (and is done with state plane i-6): refill them
+                if (tid == 0 && i + PD < niter) issue_tma(i + PD, (PH + PD) % DT);
+            }
             const int par_w = i & 1, par_r = par_w ^ 1;
             float4 out[RY];
             uint2 rout[RY];
@@ -480,8 +576,8 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                 // rows of the neighbouring threads (centre plane): fetched only by the paths that evaluate the bracket
                 float4 above, below;
                 auto load_rows = [&]() {
-                    above = exch[((k * 2 + par_r) * 2 + 1) * NT + up_tid];
-                    below = exch[((k * 2 + par_r) * 2 + 0) * NT + dn_tid];
+                    above = exch[(k * 2 + par_r) * 2 * NT + up_idx];
+                    below = exch[(k * 2 + par_r) * 2 * NT + dn_idx];
                 };
                 float mx = 0.f;                            // max |theta'| over this thread's voxels
                 float4 o[RY];
@@ -595,12 +691,13 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                     // rfa_advance() in full, two voxels per instruction (o - t and d - bv as exact-product FMAs)
                     const u64 neg1 = pk(-1.0f, -1.0f), mg = pk(RFA_COMP_MAGIC, RFA_COMP_MAGIC), nmg = pk(-RFA_COMP_MAGIC, -RFA_COMP_MAGIC);
                     const unsigned plc = (unsigned)rfa_reflect(z0 - S + i - 1, P.nz) * plane4;   // level-0 centre plane
+                    if (k == 0) ++hot_planes;
                     load_rows();
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
                         float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (hotq[k][CE]) {
-                            if (k == 0) ri = unpack_h4(__ldg(rin2 + (plc + row_src[r])));
+                            if (k == 0) ri = unpack_h4(C::RESPF ? resq[(((i & 1) ^ 1) * RY + r) * NT + tid] : __ldg(rin2 + (plc + row_src[r])));
                             else if (rvq[k][CE]) ri = unpack_h4(rsm[(((k > 0 ? k - 1 : 0) * 2 + par_r) * RY + r) * NT + tid]);
                         }
                         u64 a01, a23, n01, n23, q01, q23, t01, t23, g01, g23;
@@ -659,7 +756,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                         if (write_res) rout2[pl + row_dst[r]] = rout[r];
                         const unsigned bits = (nb_out >> (4 * r)) & 0xfu;
                         if (bits) {
-                            const uint32_t w = ringS[(sS * NT + tid) * RY + r];
+                            const uint32_t w = ringS[s_idx(sS, r)];
                             const uint32_t nw = w | ((bits & 1u) << 7) | ((bits & 2u) << 14) | ((bits & 4u) << 21) |
                                                 ((bits & 8u) << 28);
                             if (nw != w) st4[pl + row_dst[r]] = nw;
@@ -700,8 +797,12 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const RfaTbPa
                     rvq[k][0] = rvq[k][1];
                     rvq[k][1] = rvq[k][2];
                 }
+                coldq0[0] = coldq0[1];
+                coldq0[1] = coldq0[2];
             }
         }
+        // feedback for the host's choice of the RPF variant: one atomic per warp and item, only where something was hot
+        if (hot_planes != 0u && (tid & 31) == 0) atomicAdd(P.hot_ctr, (unsigned long long)hot_planes);
     }
 }
 
@@ -796,17 +897,24 @@ cudaError_t rfa_launch_plain(const RfaGrid &g, const float *tin, float *tout, co
     return cudaGetLastError();
 }
 
-template <int S, bool CONS, int SHAPE, bool HC = false>
+template <int S, bool CONS, int SHAPE, bool HC = false, bool TMA = false, bool RPF = false>
 struct TbKernel {
     static constexpr RfaTbShape sh = RFA_TB_SHAPE[SHAPE][S];
-    using C = TbCfg<S, sh.tx, sh.ty, sh.ry, CONS>;
-    static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb, CONS, HC>; }
+    using C = TbCfg<S, sh.tx, sh.ty, sh.ry, CONS, TMA, RPF>;
+    static auto get() { return rfa_blocked_kernel<S, sh.tx, sh.ty, sh.ry, sh.minb, CONS, HC, TMA, RPF>; }
 };
 
-template <int S, bool CONS, int SHAPE, bool HC>
+// the TMA variant exists for the Eq. 12 kernels with 2 or 3 fused steps (the ones the planner picks by default), the
+// residual-prefetch variant for 2 and 3 fused steps (with TMA staging: 2)
+template <int S, bool CONS>
+constexpr bool rfa_has_tma() { return !CONS && (S == 2 || S == 3); }
+template <int S, bool TMA>
+constexpr bool rfa_has_rpf() { return TMA ? S == 2 : (S == 2 || S == 3); }
+
+template <int S, bool CONS, int SHAPE, bool HC, bool TMA, bool RPF>
 static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_t st)
 {
-    using K = TbKernel<S, CONS, SHAPE, HC>;
+    using K = TbKernel<S, CONS, SHAPE, HC, TMA, RPF>;
     auto kern = K::get();
     // the dynamic shared-memory opt-in is a per-DEVICE function attribute: remember it per device ordinal
     static std::atomic<bool> attr_set[RFA_MAX_DEVICES];
@@ -822,23 +930,49 @@ static cudaError_t launch_blocked_sc(const RfaTbParams &p, int grid, cudaStream_
     return cudaGetLastError();
 }
 
-template <int S>
-static cudaError_t launch_blocked_s(const RfaTbParams &p, int shape, int grid, cudaStream_t st)
+template <int S, bool CONS, int SHAPE, bool TMA>
+static cudaError_t launch_blocked_r(const RfaTbParams &p, int grid, cudaStream_t st)
 {
-    const bool cons = p.kap != nullptr, hc = p.held_copy != 0;
-    if (shape == 0) {
-        if (cons) return hc ? launch_blocked_sc<S, true, 0, true>(p, grid, st) : launch_blocked_sc<S, true, 0, false>(p, grid, st);
-        return hc ? launch_blocked_sc<S, false, 0, true>(p, grid, st) : launch_blocked_sc<S, false, 0, false>(p, grid, st);
+    const bool hc = p.held_copy != 0;
+    if constexpr (rfa_has_rpf<S, TMA>()) {
+        if (p.res_prefetch) return hc ? launch_blocked_sc<S, CONS, SHAPE, true, TMA, true>(p, grid, st) : launch_blocked_sc<S, CONS, SHAPE, false, TMA, true>(p, grid, st);
     }
-    if (cons) return hc ? launch_blocked_sc<S, true, 1, true>(p, grid, st) : launch_blocked_sc<S, true, 1, false>(p, grid, st);
-    return hc ? launch_blocked_sc<S, false, 1, true>(p, grid, st) : launch_blocked_sc<S, false, 1, false>(p, grid, st);
+    return hc ? launch_blocked_sc<S, CONS, SHAPE, true, TMA, false>(p, grid, st) : launch_blocked_sc<S, CONS, SHAPE, false, TMA, false>(p, grid, st);
+}
+
+template <int S, bool CONS, int SHAPE>
+static cudaError_t launch_blocked_v(const RfaTbParams &p, int tma, int grid, cudaStream_t st)
+{
+    if constexpr (rfa_has_tma<S, CONS>()) {
+        if (tma) return launch_blocked_r<S, CONS, SHAPE, true>(p, grid, st);
+    } else {
+        if (tma) return cudaErrorInvalidValue;
+    }
+    return launch_blocked_r<S, CONS, SHAPE, false>(p, grid, st);
+}
+
+template <int S>
+static cudaError_t launch_blocked_s(const RfaTbParams &p, int shape, int tma, int grid, cudaStream_t st)
+{
+    const bool cons = p.kap != nullptr;
+    if (shape == 0) return cons ? launch_blocked_v<S, true, 0>(p, tma, grid, st) : launch_blocked_v<S, false, 0>(p, tma, grid, st);
+    return cons ? launch_blocked_v<S, true, 1>(p, tma, grid, st) : launch_blocked_v<S, false, 1>(p, tma, grid, st);
 }
 
 cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const float *tin, float *tout,
                                const void *rin, void *rout, uint8_t *state, const float *tables, const float *kap,
-                               cudaStream_t st)
+                               const RfaTensorMap *map_theta_in, const RfaTensorMap *map_state, int res_prefetch,
+                               unsigned long long *hot_ctr, cudaStream_t st)
 {
-    RfaTbParams p;
+    RfaTbParams p{};
+    if (plan.tma) {
+        if (!map_theta_in || !map_state || kap) return cudaErrorInvalidValue;
+        p.tm_theta = *map_theta_in;
+        p.tm_state = *map_state;
+    }
+    if (!hot_ctr) return cudaErrorInvalidValue;
+    p.res_prefetch = res_prefetch;
+    p.hot_ctr = hot_ctr;
     p.kap = kap;
     p.tin = tin;
     p.tout = tout;
@@ -862,18 +996,20 @@ cudaError_t rfa_launch_blocked(const RfaGrid &g, const RfaTbPlan &plan, const fl
     p.n_items = plan.n_items;
     p.held_copy = g.held_copy;
     switch (plan.fused) {
-    case 1: return launch_blocked_s<1>(p, plan.shape, plan.grid, st);
-    case 2: return launch_blocked_s<2>(p, plan.shape, plan.grid, st);
-    case 3: return launch_blocked_s<3>(p, plan.shape, plan.grid, st);
-    case 4: return launch_blocked_s<4>(p, plan.shape, plan.grid, st);
+    case 1: return launch_blocked_s<1>(p, plan.shape, plan.tma, plan.grid, st);
+    case 2: return launch_blocked_s<2>(p, plan.shape, plan.tma, plan.grid, st);
+    case 3: return launch_blocked_s<3>(p, plan.shape, plan.tma, plan.grid, st);
+    case 4: return launch_blocked_s<4>(p, plan.shape, plan.tma, plan.grid, st);
     default: return cudaErrorInvalidValue;
     }
 }
 
-template <int S, int SHAPE, bool CONS>
+// occupancy of the variant with the largest shared-memory footprint (residual prefetch where it exists): the plan
+// must hold for either choice of RPF
+template <int S, int SHAPE, bool CONS, bool TMA>
 static int resident_s()
 {
-    using K = TbKernel<S, CONS, SHAPE>;
+    using K = TbKernel<S, CONS, SHAPE, false, TMA, rfa_has_rpf<S, TMA>()>;
     auto kern = K::get();
     int dev = 0, sms = 0, occ = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;
@@ -889,19 +1025,38 @@ static int resident_s()
 }
 
 template <int S>
-static int resident_sc(int shape, int cons)
+static int resident_sc(int shape, int cons, int tma)
 {
-    if (shape == 0) return cons ? resident_s<S, 0, true>() : resident_s<S, 0, false>();
-    return cons ? resident_s<S, 1, true>() : resident_s<S, 1, false>();
+    if (tma) {
+        if constexpr (rfa_has_tma<S, false>()) {
+            if (cons) return 0;
+            return shape == 0 ? resident_s<S, 0, false, true>() : resident_s<S, 1, false, true>();
+        } else {
+            return 0;
+        }
+    }
+    if (shape == 0) return cons ? resident_s<S, 0, true, false>() : resident_s<S, 0, false, false>();
+    return cons ? resident_s<S, 1, true, false>() : resident_s<S, 1, false, false>();
 }
 
-int rfa_blocked_resident_ctas(int fused, int shape, int cons)
+int rfa_blocked_resident_ctas(int fused, int shape, int cons, int tma)
 {
     switch (fused) {
-    case 1: return resident_sc<1>(shape, cons);
-    case 2: return resident_sc<2>(shape, cons);
-    case 3: return resident_sc<3>(shape, cons);
-    case 4: return resident_sc<4>(shape, cons);
+    case 1: return resident_sc<1>(shape, cons, tma);
+    case 2: return resident_sc<2>(shape, cons, tma);
+    case 3: return resident_sc<3>(shape, cons, tma);
+    case 4: return resident_sc<4>(shape, cons, tma);
     default: return 0;
     }
+}
+
+// does a residual-prefetch variant exist for this plan?
+int rfa_blocked_has_prefetch(int fused, int tma) { return tma ? fused == 2 : (fused == 2 || fused == 3); }
+
+// tile of the blocked kernel for `fused` steps and `shape`: the box of its TMA variant's tensor maps
+void rfa_blocked_tile(int fused, int shape, int *bx, int *by)
+{
+    // (the box of the state volume is 16 bytes wider than bx: TbCfg::SROW)
+    *bx = 4 * RFA_TB_SHAPE[shape][fused].tx;
+    *by = RFA_TB_SHAPE[shape][fused].ry * RFA_TB_SHAPE[shape][fused].ty;
 }

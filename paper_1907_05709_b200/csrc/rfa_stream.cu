@@ -24,44 +24,7 @@
 
 #include "rfa_internal.h"
 #include "rfa_packed.cuh"
-
-// ------------------------------------------------------------------------------------------------
-// mbarrier / bulk tensor copy (PTX; no CUTLASS)
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(void *smem_dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2)
-{
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
-                     smem_u32(smem_dst)),
-                 "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
-                 : "memory");
-}
+#include "rfa_tma.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // kernel
@@ -136,7 +99,7 @@ __global__ void __launch_bounds__(32 * RFA_STREAM_NW, RFA_STREAM_MINB)
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], NW);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
 
@@ -452,31 +415,29 @@ using SCfg = StreamCfg<RFA_STREAM_RY, RFA_STREAM_D>;
 static_assert(sizeof(RfaTensorMap) == sizeof(CUtensorMap), "RfaTensorMap must hold a CUtensorMap");
 static_assert(SCfg::BY == RFA_STREAM_BY, "tile height");
 
-// tensor maps of one fp32 image and of the packed state volume, both seen as (nx, ny, nz * batch)
-bool rfa_stream_make_maps(const RfaGrid &g, const float *theta, const uint8_t *state, RfaTensorMap *map_theta, RfaTensorMap *map_state)
+// tensor map of one fp32 image (elem_bytes 4) or of the packed state volume (elem_bytes 1), seen as (nx, ny, nz * batch),
+// with a box of box_x x box_y x 1 elements
+bool rfa_make_tile_map(const RfaGrid &g, const void *base, int elem_bytes, int box_x, int box_y, RfaTensorMap *out)
 {
     EncodeTiledFn enc = encode_fn();
-    if (!enc) return false;
+    if (!enc || !out || !base) return false;
     if ((g.nx % 16) != 0) return false;                     // row pitch of the byte volume must be a multiple of 16 bytes
     if ((long long)g.nz * g.batch > 0x7fffffffLL) return false;
+    if (box_x < 1 || box_x > 256 || box_y < 1 || box_y > 256 || (box_x * elem_bytes) % 16 != 0) return false;
     const cuuint64_t dims[3] = {(cuuint64_t)g.nx, (cuuint64_t)g.ny, (cuuint64_t)g.nz * g.batch};
     const cuuint32_t estr[3] = {1, 1, 1};
-    if (map_theta) {
-        const cuuint64_t str[2] = {(cuuint64_t)g.nx * 4, (cuuint64_t)g.nx * g.ny * 4};
-        const cuuint32_t box[3] = {(cuuint32_t)(SCfg::ROW4 * 4), (cuuint32_t)(SCfg::BY + 2), 1};
-        if (enc(reinterpret_cast<CUtensorMap *>(map_theta), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(theta), dims, str, box, estr,
-                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-            return false;
-    }
-    if (map_state) {
-        const cuuint64_t str[2] = {(cuuint64_t)g.nx, (cuuint64_t)g.nx * g.ny};
-        const cuuint32_t box[3] = {(cuuint32_t)SCfg::BX, (cuuint32_t)SCfg::BY, 1};
-        if (enc(reinterpret_cast<CUtensorMap *>(map_state), CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(state), dims, str, box, estr,
-                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-            return false;
-    }
+    const cuuint64_t str[2] = {(cuuint64_t)g.nx * elem_bytes, (cuuint64_t)g.nx * g.ny * elem_bytes};
+    const cuuint32_t box[3] = {(cuuint32_t)box_x, (cuuint32_t)box_y, 1};
+    return enc(reinterpret_cast<CUtensorMap *>(out), elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 3,
+               const_cast<void *>(base), dims, str, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// the two maps of the one-step kernel: the fp32 tile with its halo, the state tile without
+bool rfa_stream_make_maps(const RfaGrid &g, const float *theta, const uint8_t *state, RfaTensorMap *map_theta, RfaTensorMap *map_state)
+{
+    if (map_theta && !rfa_make_tile_map(g, theta, 4, SCfg::ROW4 * 4, SCfg::BY + 2, map_theta)) return false;
+    if (map_state && !rfa_make_tile_map(g, state, 1, SCfg::BX, SCfg::BY, map_state)) return false;
     return true;
 }
 

@@ -135,3 +135,20 @@ def test_blocked_plan_rejects_unsupported_grids(lib):
     assert binding.plan_query((4096, 4096, 512), 1, 3, 296)["ok"] == 0  # 8.6e9 voxels: beyond 32-bit float4 offsets
     assert binding.plan_query((2048, 2048, 1024), 1, 3, 296)["ok"] == 1
     assert binding.plan_query((44, 38, 29), 1, 5, 148)["ok"] == 0
+
+
+def test_plan_of_the_tma_staged_variant(lib):
+    """RFA_STAGING_TMA: 2 or 3 fused steps, nx % 16 == 0, ny even; its tiles start a multiple of two rows above the grid, so
+    at 3 fused steps the first tile owns one row less (tiles_y = ceil((ny + 1) / 26) for the 64 x 32 tile)."""
+    TMA = binding.STAGING_TMA
+    p = binding.plan_query((512, 512, 256), 1, 3, 296, TMA)
+    assert p["ok"] == 1 and (p["bx"], p["by"], p["tiles_x"], p["tiles_y"]) == (64, 32, 9, 20)
+    assert binding.plan_query((64, 26, 40), 1, 3, 296)["tiles_y"] == 1          # cp.async: 26 rows fit one tile ...
+    assert binding.plan_query((64, 26, 40), 1, 3, 296, TMA)["tiles_y"] == 2     # ... TMA: one halo row more
+    assert binding.plan_query((64, 28, 40), 1, 2, 296, TMA)["tiles_y"] == 1     # two fused steps: no extra row
+    assert binding.plan_query((72, 38, 29), 1, 3, 148, TMA)["ok"] == 0          # nx % 16 != 0
+    assert binding.plan_query((80, 33, 29), 1, 3, 148, TMA)["ok"] == 0          # odd ny
+    assert binding.plan_query((80, 34, 29), 1, 1, 148, TMA)["ok"] == 0          # one step: the one-step kernel has its own TMA path
+    assert binding.plan_query((80, 34, 29), 1, 4, 148, TMA)["ok"] == 0
+    with pytest.raises(binding.RfaError):
+        binding.plan_query((80, 34, 29), 1, 3, 148, 7)

@@ -29,10 +29,14 @@ def rfa():
     return binding
 
 
-def run_gpu(rfa, w, steps, kernel=None, fused=0, scenario_list=None):
+def run_gpu(rfa, w, steps, kernel=None, fused=0, scenario_list=None, res_prefetch=None, cons=False):
     sim = rfa.from_workload(w)
     if kernel is not None:
         sim.configure(kernel, fused)
+    if res_prefetch is not None:
+        sim.configure_residual_prefetch(res_prefetch)
+    if cons:
+        sim.set_conduction(rfa.COND_FACE)
     sim.step(steps)
     sc = range(w.batch) if scenario_list is None else scenario_list
     T = [sim.get_temperature(b) for b in sc]
@@ -80,12 +84,78 @@ def test_ragged_parity_and_variants(rfa, oracle, case):
             assert qb["kernel"] == rfa.KERNEL_BLOCKED and qb["fused_steps"] == fused
             assert np.array_equal(Tb[0].view(np.uint32), Tp[0].view(np.uint32)), f"fused={fused} differs from plain"
             assert np.array_equal(Nb[0], Np[0])
+        # the residual-prefetch variant (fp16 residual rows of hot planes fetched one plane ahead): same bits, Eq. 12 and conservative
+        for fused in (2, 3):
+            Tr, Nr, _ = run_gpu(rfa, w, w.steps, rfa.KERNEL_BLOCKED, fused, res_prefetch=rfa.RES_PREFETCH_ON)
+            assert np.array_equal(Tr[0].view(np.uint32), Tp[0].view(np.uint32)), f"fused={fused} with residual prefetch differs from plain"
+            assert np.array_equal(Nr[0], Np[0])
+        Tc0, Nc0, _ = run_gpu(rfa, w, w.steps, rfa.KERNEL_PLAIN, cons=True)
+        Tc1, Nc1, _ = run_gpu(rfa, w, w.steps, rfa.KERNEL_BLOCKED, 3, res_prefetch=rfa.RES_PREFETCH_ON, cons=True)
+        assert np.array_equal(Tc1[0].view(np.uint32), Tc0[0].view(np.uint32)) and np.array_equal(Nc1[0], Nc0[0])
     else:
         Ta, Na, qa = run_gpu(rfa, w, w.steps, rfa.KERNEL_AUTO)
         assert qa["kernel"] == rfa.KERNEL_PLAIN     # falls back to the plain CUDA kernel, still on the GPU
         assert np.array_equal(Ta[0], Tp[0])
         with pytest.raises(rfa.RfaError):
             rfa.from_workload(w).configure(rfa.KERNEL_BLOCKED, 2)
+
+
+TMA_CASES = [
+    dict(dims=(144, 70, 21), spacing=(0.7, 0.9, 1.3), steps=37, mode=W.SRC_DIRICHLET, value=90.0, batch=1),   # 3 x 3 tiles of 64 x 32, ragged
+    dict(dims=(80, 130, 19), spacing=(1.1, 0.8, 0.9), steps=41, mode=W.SRC_POWER, value=2.0e7, batch=1),       # partial x tile, 5-6 y tiles
+    dict(dims=(16, 38, 29), spacing=(1.0, 1.0, 1.0), steps=50, mode=W.SRC_DIRICHLET, value=60.0, batch=1),     # narrower than a tile
+    dict(dims=(272, 34, 7), spacing=(0.7, 0.9, 1.3), steps=20, mode=W.SRC_DIRICHLET, value=90.0, batch=1),     # 5 x tiles, few planes
+    dict(dims=(64, 66, 23), spacing=(1.0, 1.0, 1.2), steps=33, mode=W.SRC_DIRICHLET, value=90.0, batch=3),     # batched
+]
+
+
+@pytest.mark.parametrize("case", TMA_CASES, ids=lambda c: "x".join(map(str, c["dims"])) + f"b{c['batch']}")
+def test_blocked_tma_staging_bit_identity(rfa, case):
+    """The temporally blocked kernel with its level-0 planes staged by the Tensor Memory Accelerator (RFA_STAGING_TMA: one
+    cp.async.bulk.tensor per tile plane, zero-filled outside the grid, replicate rule at the outer y faces by exchange
+    index) against the plain kernel, bit for bit: 2 and 3 fused steps, both tile shapes, both held-copy settings."""
+    w = W.ragged_phantom(dims=case["dims"], spacing=case["spacing"], steps=case["steps"], mode=case["mode"],
+                         value=case["value"], q_m=10714.0, dt=0.05, batch=case["batch"])
+    w.table["t_init"][W.KIDNEY] = 36.0
+    Tp, Np, qp = run_gpu(rfa, w, w.steps, rfa.KERNEL_PLAIN)
+    for fused in (2, 3):
+        for shape in (0, 1):
+            for hc in (0, 1):
+                sim = rfa.from_workload(w)
+                sim.configure(rfa.KERNEL_BLOCKED, fused)
+                sim.configure_tile(shape)
+                sim.configure_staging(rfa.STAGING_TMA)
+                sim.configure_held_copy(hc)
+                sim.configure_residual_prefetch(rfa.RES_PREFETCH_ON if hc else rfa.RES_PREFETCH_OFF)   # exists with TMA staging at 2 fused steps
+                v = sim.query_variant()
+                assert v["residual_prefetch"] == (1 if hc and fused == 2 else 0)
+                assert v["staging"] == rfa.STAGING_TMA and v["fused_steps"] == fused and v["held_copy"] == hc
+                assert (v["tile_bx"], v["tile_by"]) == ((64, 32), (128, 16))[shape]
+                sim.step(w.steps)
+                for b in range(w.batch):
+                    T, N = sim.get_temperature(b), sim.get_necrosis(b)
+                    assert np.array_equal(T.view(np.uint32), Tp[b].view(np.uint32)), \
+                        f"TMA-staged blocked kernel differs from plain (fused {fused}, shape {shape}, hc {hc}, scenario {b})"
+                    assert np.array_equal(N, Np[b])
+                sim.close()
+    # default staging: TMA with the 128 x 16 tile, cp.async with the 64 x 32 tile; both can be forced
+    sim = rfa.from_workload(w)
+    sim.configure(rfa.KERNEL_BLOCKED, 3)
+    v = sim.query_variant()
+    assert v["staging"] == (rfa.STAGING_TMA if v["tile_bx"] == 128 else rfa.STAGING_CP_ASYNC)
+    sim.configure_staging(rfa.STAGING_CP_ASYNC)
+    assert sim.query_variant()["staging"] == rfa.STAGING_CP_ASYNC
+    sim.step(w.steps)
+    assert np.array_equal(sim.get_temperature(0).view(np.uint32), Tp[0].view(np.uint32))
+    sim.close()
+    # no TMA variant: odd ny, nx % 16 != 0
+    for dims in ((272, 33, 5), (136, 70, 21)):
+        sim = rfa.from_workload(W.ragged_phantom(dims=dims, steps=3))
+        sim.configure(rfa.KERNEL_BLOCKED, 3)
+        assert sim.query_variant()["staging"] == rfa.STAGING_CP_ASYNC
+        with pytest.raises(rfa.RfaError):
+            sim.configure_staging(rfa.STAGING_TMA)
+        sim.close()
 
 
 STREAM_CASES = [
@@ -788,3 +858,26 @@ def test_full_size_short_run_fieldwide_vs_live_oracle(rfa, oracle, name, conserv
     err, n_band = compare(sim.get_temperature(0), sim.get_necrosis(0), osim)
     print(f"{name}{' (conservative)' if conservative else ''}: 7 steps, field max|dT| {err:.2e} over {w.n_voxels} voxels")
     sim.close()
+
+
+def test_residual_prefetch_switches_on_by_itself(rfa):
+    """AUTO mode: the kernels count the warp-planes that take the compensated path; once the library has seen that a few
+    percent of them do, it launches the residual-prefetch variant (no synchronisation involved), and the field is the same
+    bit for bit as with the variant forced off."""
+    w = W.ragged_phantom(dims=(144, 70, 41), spacing=(0.7, 0.9, 1.3), steps=600, mode=W.SRC_POWER, value=4.0e7, dt=0.05)
+    sims = {}
+    for mode in (rfa.RES_PREFETCH_AUTO, rfa.RES_PREFETCH_OFF):
+        sim = rfa.from_workload(w)
+        sim.configure(rfa.KERNEL_BLOCKED, 3)
+        sim.configure_residual_prefetch(mode)
+        for _ in range(6):                      # several calls: the feedback is looked at when a later launch is issued
+            sim.step(100)
+            sim.synchronize()
+        sims[mode] = (sim.get_temperature(0), sim.hot_fraction(), sim.query_variant())
+        sim.close()
+    Ta, ha, va = sims[rfa.RES_PREFETCH_AUTO]
+    To, ho, vo = sims[rfa.RES_PREFETCH_OFF]
+    assert np.array_equal(Ta.view(np.uint32), To.view(np.uint32))
+    assert ha["hot_fraction"] > 0.004, ha      # a power source of 4e7 W/m3 warms a good part of this small grid by >= 1 C
+    assert ha["residual_prefetch"] == 1 and va["residual_prefetch"] == 1
+    assert ho["residual_prefetch"] == 0 and vo["residual_prefetch"] == 0
