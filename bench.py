@@ -545,8 +545,10 @@ def run_record(args):
 
 def run_render(args):
     """Row f4 (headless view of the heat zone) on the C4 volume: K frames of 512 x 512 pixels, oblique view,
-    0.5 mm steps.  Reported as frame time and trilinear samples per second (no roofline: the kernel is a
-    gather through L2 with fp64 ray arithmetic, neither an HBM stream nor a contraction)."""
+    0.5 mm steps.  Reported as frame time (host images), kernel time (device images) and trilinear samples per second.
+    The kernel is a gather: eight 4-byte loads per sample that counts, served by L1 (ncu: 95 % hit rate).  Its roofline is
+    the L1 request rate: one warp-wide load per SM and clock if the 32 addresses fell into one 128-byte line; the oblique
+    view needs about five lines per load (ncu), which is what bounds it (profiles/r2_view_kernels_ncu.md)."""
     import torch
     from paper_1907_05709_b200 import binding, workloads as W
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
@@ -566,15 +568,47 @@ def run_render(args):
         e1.record(stream)
         e1.synchronize()
         ms = float(e0.elapsed_time(e1)) / K
+        # kernel alone: both images stay on the device
+        t_dev = torch.empty(512 * 512, dtype=torch.float32, device=dev)
+        d_dev = torch.empty(512 * 512, dtype=torch.float32, device=dev)
+        sim.render_zone(0, (1, 2, 3), (0, 1, 0), 512, 512, 0.7, 0.5, 42.5, tmax=t_dev, depth=d_dev)
+        e0.record(stream)
+        for _ in range(K):
+            sim.render_zone(0, (1, 2, 3), (0, 1, 0), 512, 512, 0.7, 0.5, 42.5, tmax=t_dev, depth=d_dev)
+        e1.record(stream)
+        e1.synchronize()
+        ms_dev = float(e0.elapsed_time(e1)) / K
         sim.close()
     ext = [n * h for n, h in zip(w.dims, w.spacing_mm)]
     ns = int(np.floor(np.sqrt(sum(e * e for e in ext)) / 0.5)) + 1
+    # samples that count (inside the box of voxel centres), from the geometry of the view (include/rfa.h: rfa_render_zone)
+    wv = np.array([1.0, 2.0, 3.0]); wv /= np.linalg.norm(wv)
+    e1v = np.cross(np.array([0.0, 1.0, 0.0]), wv); e1v /= np.linalg.norm(e1v)
+    e2v = np.cross(wv, e1v)
+    c = 0.5 * np.array(ext); R = 0.5 * float(np.sqrt(sum(e * e for e in ext)))
+    uu = (np.arange(512) - 255.5) * 0.7
+    o = c[None, None, :] + uu[None, :, None] * e1v + uu[:, None, None] * e2v - R * wv
+    h = np.array(w.spacing_mm, dtype=np.float64); nn = np.array(w.dims, dtype=np.float64)
+    q0, dq = o / h - 0.5, 0.5 * wv / h
+    lo = np.zeros((512, 512)); hi = np.full((512, 512), ns - 1.0)
+    for a in range(3):
+        t0, t1 = (0.0 - q0[..., a]) / dq[a], (nn[a] - 1.0 - q0[..., a]) / dq[a]
+        lo, hi = np.maximum(lo, np.minimum(t0, t1)), np.minimum(hi, np.maximum(t0, t1))
+    inside = float(np.maximum(np.floor(hi) - np.ceil(lo) + 1.0, 0.0).sum())
+    sm_count, sm_hz = 148, 1.965e9
+    req = inside * 8 / 32 / (ms_dev * 1e-3)                 # warp-wide gather loads per second
+    roof = {"bound": "l1", "achieved": req / 1e9, "peak": sm_count * sm_hz / 1e9, "unit": "G warp-wide loads/s",
+            "frac": req / (sm_count * sm_hz), "traffic": None,
+            "peak_source": "148 SMs x 1965 MHz x one 128-byte L1 line per clock (B200_PROFILING.md unit counts and clocks); a load "
+                           "of this view touches ~5 lines (ncu), so the L1 is ~5x busier than frac says",
+            "kernel": "rfa_render_kernel", "kernel_ms": ms_dev, "samples_inside_box": inside,
+            "gsamples_inside_per_s": inside / (ms_dev * 1e-3) / 1e9}
     print(json.dumps({"metric": "frames/s (heat-zone view, 512x512, host images)", "value": 1e3 / ms, "unit": "frames/s",
                       "n_gpus": 1, "steps": K, "warmup": 3, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                       "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                       "config": {"workload": w.name + " view", "dims": list(w.dims), "image": [512, 512], "step_mm": 0.5,
                                  "samples_per_ray": ns, "visible_pixels": int((depth >= 0).sum())},
-                      "gsamples_per_s": 512 * 512 * ns / (ms * 1e-3) / 1e9, "roofline": None, "gpu_launches": K}), flush=True)
+                      "gsamples_per_s": 512 * 512 * ns / (ms * 1e-3) / 1e9, "roofline": roof, "gpu_launches": 2 * K + 1}), flush=True)
     return 0
 
 

@@ -310,12 +310,15 @@ class RfaSim:
         return out
 
     def render_zone(self, scenario: int, direction, up, width: int, height: int, pixel_mm: float, step_mm: float,
-                    iso_c: float = 42.5, want_depth: bool = True):
-        """Orthographic ray-march of the heat zone: (tmax image, depth-of-isotherm image), each (height, width)"""
+                    iso_c: float = 42.5, want_depth: bool = True, tmax=None, depth=None):
+        """Orthographic ray-march of the heat zone: (tmax image, depth-of-isotherm image), each (height, width).
+        ``tmax`` / ``depth``: optional caller buffers of width*height floats (numpy or CUDA tensors); returned as given."""
         v = RfaView((ctypes.c_float * 3)(*[float(x) for x in direction]), (ctypes.c_float * 3)(*[float(x) for x in up]),
                     int(width), int(height), float(pixel_mm), float(step_mm), float(iso_c))
-        tmax = np.empty((height, width), dtype=np.float32)
-        depth = np.empty((height, width), dtype=np.float32) if want_depth else None
+        if tmax is None:
+            tmax = np.empty((height, width), dtype=np.float32)
+        if depth is None and want_depth:
+            depth = np.empty((height, width), dtype=np.float32)
         _check(self._lib.rfa_render_zone(self._handle, int(scenario), ctypes.byref(v), _ptr(tmax),
                                          _ptr(depth) if depth is not None else None))
         return tmax, depth
