@@ -161,7 +161,7 @@ static bool ws_layout(const int dims[3], int batch, WsLayout &L)
     L.scratch = off;
     off = align256(off + nvox * 4);
     L.counters = off;
-    off = align256(off + 256);
+    off = align256(off + 256 + 256 * 8);                     // 32 counters + the 256 bins of the label histogram
     L.total = off;
     return true;
 }
@@ -443,21 +443,17 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     for (int l = 0; l < n_tissue; ++l)
         if (!tissue_ok(table[l])) return fail(RFA_E_INVALID, "tissue row %d: non-finite or non-positive constants", l);
     const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];
-    // one pass over the host label volume: histogram of the label ids (range check, held volume)
-    size_t hist[256] = {0};
     {
-        size_t h4[4][256] = {{0}};                           // four independent counters: no store-to-load chain
+        // range check of the label ids before anything touches the device: a plain byte maximum (the compiler vectorises
+        // it; the histogram that also yields the held share is taken on the device after the upload)
+        unsigned char m[64] = {0};
         size_t v = 0;
-        for (; v + 4 <= nvox; v += 4) {
-            h4[0][labels[v]]++;
-            h4[1][labels[v + 1]]++;
-            h4[2][labels[v + 2]]++;
-            h4[3][labels[v + 3]]++;
-        }
-        for (; v < nvox; ++v) h4[0][labels[v]]++;
-        for (int l = 0; l < 256; ++l) hist[l] = h4[0][l] + h4[1][l] + h4[2][l] + h4[3][l];
-        for (int l = 255; l >= n_tissue; --l)
-            if (hist[l]) return fail(RFA_E_INVALID, "label id %d >= n_tissue %d", l, n_tissue);
+        for (; v + 64 <= nvox; v += 64)
+            for (int c = 0; c < 64; ++c) m[c] = labels[v + c] > m[c] ? labels[v + c] : m[c];
+        unsigned mx = 0;
+        for (; v < nvox; ++v) mx = labels[v] > mx ? labels[v] : mx;
+        for (int c = 0; c < 64; ++c) mx = m[c] > mx ? m[c] : mx;
+        if ((int)mx >= n_tissue) return fail(RFA_E_INVALID, "label id %u >= n_tissue %d", mx, n_tissue);
     }
     const double stab = rfa_stability_number(spacing_mm, table, n_tissue, dt_s);
     if (stab < 0) return fail(RFA_E_INVALID, "invalid constants");
@@ -498,16 +494,6 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
     s->dt = dt_s;
     s->t_blood = t_blood_c;
     s->g.t_blood = t_blood_c;
-    {
-        // Held-copy kernel variant (warps whose voxels are all held copy their rows instead of evaluating the
-        // bracket; bit-identical): worth its extra vote per level only where a good part of the volume is held
-        // (the air around the body in C4: +11 %; -7 % on the 128^3 phantoms without it).  rfa_configure_held_copy overrides.
-        size_t n_held = 0;
-        for (int l = 0; l < n_tissue; ++l)
-            if (table[l].flags & RFA_TISSUE_HELD) n_held += hist[l];
-        s->held_copy_auto = n_held * 8 >= nvox ? 1 : 0;
-        s->g.held_copy = s->held_copy_auto;
-    }
     s->g.thr = (float)(60.0 - (double)t_blood_c);            // T >= 60 C  (R-11)
     s->table.assign(table, table + n_tissue);
     for (int l = 0; l < n_tissue; ++l)
@@ -585,6 +571,11 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
             }
         e = cudaMemcpyAsync(s->kap, kap, sizeof kap, cudaMemcpyHostToDevice, s->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "face table upload"); break; }
+        // histogram of the label ids, on the device (held share below)
+        unsigned long long *hist_dev = s->counters + 32;
+        e = rfa_launch_label_hist(s->g, s->scratch, hist_dev, s->stream);
+        s->launches++;
+        if (e != cudaSuccess) { rc = cuda_fail(e, "label histogram"); break; }
         e = rfa_launch_init(s->g, s->scratch, theta0, kl, s->theta[0], s->resid[0], s->state, s->stream);
         s->launches++;
         if (e != cudaSuccess) { rc = cuda_fail(e, "init kernel"); break; }
@@ -592,12 +583,32 @@ extern "C" int rfa_create(rfa_sim **out, const int dims[3], const float spacing_
         if (rc != RFA_OK) break;
         make_plans(s);
         s->fused = default_fused(s);
+        unsigned long long hist[256];
+        e = cudaMemcpyAsync(hist, hist_dev, sizeof hist, cudaMemcpyDeviceToHost, s->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "histogram download"); break; }
         e = cudaStreamSynchronize(s->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "create"); break; }
+        for (int l = 255; l >= n_tissue; --l)
+            if (hist[l]) { rc = fail(RFA_E_INVALID, "label id %d >= n_tissue %d", l, n_tissue); break; }
+        if (rc != RFA_OK) break;
+        // Held-copy kernel variant (warps whose voxels are all held copy their rows instead of evaluating the
+        // bracket; bit-identical): worth its extra vote per level only where a good part of the volume is held
+        // (the air around the body in C4: +11 %; -7 % on the 128^3 phantoms without it).  rfa_configure_held_copy overrides.
+        unsigned long long n_held = 0;
+        for (int l = 0; l < n_tissue; ++l)
+            if (table[l].flags & RFA_TISSUE_HELD) n_held += hist[l];
+        s->held_copy_auto = n_held * 8 >= (unsigned long long)nvox ? 1 : 0;
+        s->g.held_copy = s->held_copy_auto;
     } while (0);
     if (rc != RFA_OK) {
+        const std::string msg = g_err;                     // keep the message of the failure, not of the clean-up
+        cudaStreamSynchronize(s->stream);
+        cudaGetLastError();
+        if (s->hot_host) cudaFreeHost(s->hot_host);
+        if (s->hot_evt) cudaEventDestroy(s->hot_evt);
         if (s->own_ws) cudaFree(s->ws);
         delete s;
+        g_err = msg;
         return rc;
     }
     *out = s;

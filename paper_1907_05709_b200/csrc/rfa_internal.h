@@ -83,6 +83,8 @@ cudaError_t rfa_launch_table(const RfaTableHost &tbl, float *dst, cudaStream_t s
 cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const float *theta0_by_label /*host, 16*/,
                             const float *k_by_label /*host, 16*/, float *theta, void *resid, uint8_t *state,
                             cudaStream_t st);
+// label histogram of the uploaded volume (256 bins, device; zeroed by the call)
+cudaError_t rfa_launch_label_hist(const RfaGrid &g, const uint8_t *labels_dev, unsigned long long *hist_dev, cudaStream_t st);
 cudaError_t rfa_launch_needle(const RfaGrid &g, int scenario, const uint8_t *mask_dev /*may be null*/, int mode,
                               float theta_value, float *theta, void *resid, uint8_t *state, cudaStream_t st);
 cudaError_t rfa_launch_set_temperature(const RfaGrid &g, int scenario, const float *t_dev, float *theta,

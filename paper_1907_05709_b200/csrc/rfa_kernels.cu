@@ -6,6 +6,7 @@
 //
 // Every stepping kernel evaluates rfa_bracket() + rfa_advance() (rfa_device.cuh) with the same operands
 // in the same order, so all variants produce bit-identical fields.
+#include <algorithm>
 #include <atomic>
 #include <cstdio>
 
@@ -86,6 +87,33 @@ __global__ void rfa_init_kernel(int nx, int ny, int nz, int batch, const uint8_t
         resid[(size_t)b * nvox + v] = __float2half_rn(0.f);
         state[(size_t)b * nvox + v] = (uint8_t)st;
     }
+}
+
+// histogram of the label ids of the uploaded volume (range check and held share in rfa_create; on the host this walk
+// over the label volume was most of rfa_create's time): 16 bytes per thread, one shared-memory histogram per block
+__global__ void rfa_label_hist_kernel(size_t nvox, const uint8_t *__restrict__ labels, unsigned long long *__restrict__ hist)
+{
+    __shared__ unsigned h[256];
+    for (int e = threadIdx.x; e < 256; e += blockDim.x) h[e] = 0u;
+    __syncthreads();
+    const size_t n16 = nvox / 16, stride = (size_t)gridDim.x * blockDim.x;
+    const uint4 *l16 = reinterpret_cast<const uint4 *>(labels);
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < n16; v += stride) {
+        const uint4 w = l16[v];
+        const unsigned ws[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            atomicAdd(&h[ws[c] & 0xffu], 1u);
+            atomicAdd(&h[(ws[c] >> 8) & 0xffu], 1u);
+            atomicAdd(&h[(ws[c] >> 16) & 0xffu], 1u);
+            atomicAdd(&h[ws[c] >> 24], 1u);
+        }
+    }
+    if (blockIdx.x == 0)
+        for (size_t v = n16 * 16 + threadIdx.x; v < nvox; v += blockDim.x) atomicAdd(&h[labels[v]], 1u);
+    __syncthreads();
+    for (int e = threadIdx.x; e < 256; e += blockDim.x)
+        if (h[e]) atomicAdd(&hist[e], (unsigned long long)h[e]);
 }
 
 // needle placement for one scenario (R-15, R-16, R-17)
@@ -828,6 +856,17 @@ cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const f
     size_t nvox = (size_t)g.nx * g.ny * g.nz;
     rfa_init_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(g.nx, g.ny, g.nz, g.batch, labels_dev, li, g.thr, theta,
                                                            (__half *)resid, state);
+    return cudaGetLastError();
+}
+
+cudaError_t rfa_launch_label_hist(const RfaGrid &g, const uint8_t *labels_dev, unsigned long long *hist_dev /*256, zeroed here*/,
+                                  cudaStream_t st)
+{
+    const size_t nvox = (size_t)g.nx * g.ny * g.nz;
+    cudaError_t e = cudaMemsetAsync(hist_dev, 0, 256 * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    const unsigned blocks = (unsigned)std::min<size_t>((nvox / 16 + 255) / 256 + 1, 148 * 8);
+    rfa_label_hist_kernel<<<blocks, 256, 0, st>>>(nvox, labels_dev, hist_dev);
     return cudaGetLastError();
 }
 
