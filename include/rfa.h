@@ -98,7 +98,7 @@ size_t rfa_workspace_bytes(const int dims[3], int batch);
 double rfa_stability_number(const float spacing_mm[3], const rfa_tissue *table, int n_tissue, float dt_s);
 
 /* Create a simulation of `batch` independent scenarios that share one label volume.
- *   dims        nx, ny, nz (> 0)
+ *   dims        nx, ny, nz (> 0; ny, nz <= 65535)
  *   spacing_mm  voxel spacing in millimetres, converted to metres internally
  *   labels      host, nx*ny*nz bytes, label ids < n_tissue
  *   table       host, n_tissue rows (<= RFA_MAX_TISSUES)
@@ -178,7 +178,8 @@ int rfa_configure_staging(rfa_sim *s, int mode);
  * DESIGN.md section 5) of planes with |T - T_a| >= 1 C are fetched one plane ahead instead of where they are used.  It pays
  * where a few percent or more of the volume is that warm and costs ~3 % where next to nothing is, so in AUTO (the default) the
  * library switches it on and off from the share of such planes that the kernels count as they run (no synchronisation:
- * the count is copied to pinned memory asynchronously and looked at when it has arrived).  All settings give bit-identical
+ * the count is copied to pinned memory asynchronously and looked at when it has arrived; in AUTO mode rfa_step stops
+ * running more than ~64 launches ahead of the device, which always has 32 launches queued).  All settings give bit-identical
  * fields.  rfa_query_hot_fraction returns the last share seen and the variant in use (either pointer may be NULL). */
 enum { RFA_RES_PREFETCH_AUTO = -1, RFA_RES_PREFETCH_OFF = 0, RFA_RES_PREFETCH_ON = 1 };
 int rfa_configure_residual_prefetch(rfa_sim *s, int mode);

@@ -139,7 +139,7 @@ static bool ws_layout(const int dims[3], int batch, WsLayout &L)
 {
     if (!dims || batch < 1) return false;
     for (int a = 0; a < 3; ++a)
-        if (dims[a] < 1) return false;
+        if (dims[a] < 1 || (a > 0 && dims[a] > 65535)) return false;   // ny, nz are grid dimensions of the set-up kernels
     const double nv = (double)dims[0] * dims[1] * dims[2];
     if (nv * batch > 1.0e11) return false;
     const size_t nvox = (size_t)dims[0] * dims[1] * dims[2];

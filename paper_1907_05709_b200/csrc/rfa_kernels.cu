@@ -64,23 +64,31 @@ __global__ void rfa_init_kernel(int nx, int ny, int nz, int batch, const uint8_t
                                 float thr, float *__restrict__ theta, __half *__restrict__ resid,
                                 uint8_t *__restrict__ state)
 {
+    // grid = (x blocks, rows, planes): no integer division per voxel
     const size_t nvox = (size_t)nx * ny * nz;
-    size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= nvox) return;
-    const int i = (int)(v % nx);
-    const int j = (int)((v / nx) % ny);
-    const int k = (int)(v / ((size_t)nx * ny));
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y, k = blockIdx.z;
+    // the per-label constants are indexed by data: from shared memory (indexed out of the parameter bank, the divergent
+    // lookups were serialised and the kernel took 3.7 ms for 67 M voxels)
+    __shared__ float sk[RFA_NLABEL], st0[RFA_NLABEL];
+    if (threadIdx.x < RFA_NLABEL) {
+        sk[threadIdx.x] = li.k[threadIdx.x];
+        st0[threadIdx.x] = li.theta0[threadIdx.x];
+    }
+    __syncthreads();
+    if (i >= nx) return;
     const size_t sy = nx, sz = (size_t)nx * ny;
+    const size_t v = (size_t)k * sz + (size_t)j * sy + i;
     unsigned l = labels[v] & RFA_ST_LABEL;
-    const float kc = li.k[l];
+    const float kc = sk[l];
     bool iface = false;
-    if (i > 0) iface |= li.k[labels[v - 1] & RFA_ST_LABEL] != kc;
-    if (i < nx - 1) iface |= li.k[labels[v + 1] & RFA_ST_LABEL] != kc;
-    if (j > 0) iface |= li.k[labels[v - sy] & RFA_ST_LABEL] != kc;
-    if (j < ny - 1) iface |= li.k[labels[v + sy] & RFA_ST_LABEL] != kc;
-    if (k > 0) iface |= li.k[labels[v - sz] & RFA_ST_LABEL] != kc;
-    if (k < nz - 1) iface |= li.k[labels[v + sz] & RFA_ST_LABEL] != kc;
-    float t = li.theta0[l];
+    if (i > 0) iface |= sk[labels[v - 1] & RFA_ST_LABEL] != kc;
+    if (i < nx - 1) iface |= sk[labels[v + 1] & RFA_ST_LABEL] != kc;
+    if (j > 0) iface |= sk[labels[v - sy] & RFA_ST_LABEL] != kc;
+    if (j < ny - 1) iface |= sk[labels[v + sy] & RFA_ST_LABEL] != kc;
+    if (k > 0) iface |= sk[labels[v - sz] & RFA_ST_LABEL] != kc;
+    if (k < nz - 1) iface |= sk[labels[v + sz] & RFA_ST_LABEL] != kc;
+    float t = st0[l];
     unsigned st = l | (iface ? RFA_ST_IFACE : 0u) | (t >= thr ? RFA_ST_NECRO : 0u);
     for (int b = 0; b < batch; ++b) {
         theta[(size_t)b * nvox + v] = t;
@@ -794,7 +802,8 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             }
         };
 
-        if constexpr (!CONS) {
+        // (the TMA variant indexes its ring by the iteration number mod 3 = the unrolled body: always unrolled)
+        if constexpr (TMA || (!CONS && !(HELDCOPY && S >= 3))) {
             for (int i = 0;;) {
                 body(IC<0>{}, i);
                 if (++i >= niter) break;
@@ -807,7 +816,10 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             // The conservative variant carries the face-term code in every mixed / hot path; unrolled three times
             // it is 185 KB of SASS and stalls on instruction fetch (ncu: no_instruction 1.47 per issue, 380 GVox/s).
             // One body and an explicit rotation of the plane registers instead: a third of the code, 48 moves more
-            // (446 GVox/s; the same rotation costs the Eq. 12 variant 4.5 %, so that one stays unrolled).
+            // (446 GVox/s).  The same holds for the held-copy variant at three fused steps, whose warps run two different
+            // paths side by side (copy / bracket): unrolled, no_instruction is its largest stall (1.36 per issue) and C4
+            // runs 786 GVox/s, rotated 806.  Without held-copy (no_instruction 0.47) and at two fused steps the unrolled
+            // body wins (C4, S = 2: 728 vs 713), so those stay unrolled.
 #pragma unroll 1
             for (int i = 0; i < niter; ++i) {
                 body(IC<2>{}, i);                          // arrival in slot 2, centre 1, previous 0
@@ -853,9 +865,10 @@ cudaError_t rfa_launch_init(const RfaGrid &g, const uint8_t *labels_dev, const f
         li.theta0[i] = theta0_by_label[i];
         li.k[i] = k_by_label[i];
     }
-    size_t nvox = (size_t)g.nx * g.ny * g.nz;
-    rfa_init_kernel<<<blocks_for(nvox, 256), 256, 0, st>>>(g.nx, g.ny, g.nz, g.batch, labels_dev, li, g.thr, theta,
-                                                           (__half *)resid, state);
+    if (g.ny > 65535 || g.nz > 65535) return cudaErrorInvalidValue;
+    const int bs = g.nx >= 256 ? 256 : (g.nx >= 128 ? 128 : 64);
+    const dim3 grid((unsigned)((g.nx + bs - 1) / bs), (unsigned)g.ny, (unsigned)g.nz);
+    rfa_init_kernel<<<grid, bs, 0, st>>>(g.nx, g.ny, g.nz, g.batch, labels_dev, li, g.thr, theta, (__half *)resid, state);
     return cudaGetLastError();
 }
 
