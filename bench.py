@@ -42,8 +42,9 @@ METRIC = "GVoxel-updates/s"
 # Algorithmic bytes per voxel per launch of the stepping kernel.  SURVEY.md 8(d) counts
 # 4 B theta read + 4 B theta write + 1 B label/flag byte + 1 B necrosis byte = 10 B, i.e. (8+2)/S per voxel-update with
 # S fused steps; that is the figure roofline.frac is taken on.  This build keeps the necrosis bit inside the state
-# byte (no second byte) but writes a 2-B fp16 residual image for the compensated accumulation: 4 + 4 + 1 + 2 = 11 B
-# is what the kernel itself must move, reported beside it as frac_11B.
+# byte (no second byte) and has a 2-B fp16 residual image for the compensated accumulation: 4 + 4 + 1 + 2 = 11 B was
+# round 1's own count, reported beside it as frac_11B (since round 2 the residual is written for hot rows only: the
+# measured DRAM traffic is 8.5-8.8 B per voxel per launch, the `traffic` key).
 BYTES_SURVEY = {"theta_read": 4.0, "theta_write": 4.0, "label_byte": 1.0, "necrosis_byte": 1.0}
 BYTES_BUILD = {"theta_read": 4.0, "theta_write": 4.0, "state_byte_read": 1.0, "residual_fp16_write": 2.0}
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel, from the `ncu --set full`
@@ -51,6 +52,17 @@ BYTES_BUILD = {"theta_read": 4.0, "theta_write": 4.0, "state_byte_read": 1.0, "r
 # held-copy / conduction): a run whose variant has no capture prints "traffic": null.
 NCU_TRAFFIC = {
     # variant: (bytes per launch, profile file)
+    "C4/S3/64x32/hc1/eq12": (587.2e6, "profiles/r2_blocked_s3_final_ncu.md"),
+    "C4/S3/64x32/hc0/eq12": (577.6e6, "profiles/r2_variants_ncu.md"),
+    "C4/S2/64x32/hc1/eq12": (577.3e6, "profiles/r2_variants_ncu.md"),
+    "C4/S1/128x16/hc1/eq12/tma": (569.1e6, "profiles/r2_variants_ncu.md"),
+    "C4/S1/128x16/hc0/eq12/tma": (569.1e6, "profiles/r2_variants_ncu.md"),
+    "C3/S3/64x32/hc0/eq12/rpf": (120.6e6, "profiles/r2_blocked_ab_ncu.md"),
+    "C3/S3/64x32/hc0/eq12": (120.6e6, "profiles/r2_blocked_ab_ncu.md"),
+    "C5/S2/128x16/hc0/eq12/tma": (1200.1e6, "profiles/r2_blocked_ab_ncu.md"),
+    "C4/S3/64x32/hc1/face": (641.8e6, "profiles/r2_variants_ncu.md"),
+    "C4F/S3/64x32/hc1/face/rpf": (870.9e6, "profiles/r2_blocked_ab_ncu.md"),
+    "C4/plain": (840.3e6, "profiles/r2_variants_ncu.md"),
 }
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
