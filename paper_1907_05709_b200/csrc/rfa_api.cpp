@@ -410,8 +410,9 @@ static void make_plans(rfa_sim *s)
                 res_tma[sh] = (want && m == 0 && blk_maps[sh] && s->staging != RFA_STAGING_CP_ASYNC) ? rfa_blocked_resident_ctas(f, sh, m, 1) : 0;
             }
             // AUTO: the TMA-staged variant where it measured faster on the B200 -- the 128 x 16 tile (C5: 684 -> 704 GVox/s);
-            // with the 64 x 32 tile the elected thread's issue sequence sits on the critical path of the per-plane barrier
-            // and the per-thread cp.async variant wins (C4: 783 vs 707), profiles/r2_blocked_tma_vs_cpasync.md
+            // with the 64 x 32 tile it executes more instructions than it saves (row-major state tile: two 4-byte loads per
+            // level instead of one 8-byte load, more index arithmetic) and the per-thread cp.async variant wins
+            // (C4: 783 vs 707), profiles/r2_blocked_ab_ncu.md
             const RfaTbPlan pc = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, s->resident[m][f], 0);
             const RfaTbPlan pt = rfa_plan_blocked(s->g.nx, s->g.ny, s->g.nz, s->g.batch, f, res_tma, 1);
             const bool take_tma = pt.ok && (s->staging == RFA_STAGING_TMA || !pc.ok || (pt.shape == 1 && pc.shape == 1));
