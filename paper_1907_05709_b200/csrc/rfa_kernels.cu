@@ -520,14 +520,15 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             }
         }
 
-        // one plane iteration; PH = i mod 3 selects the register slots at compile time
-        auto body = [&](auto ph, const int i) {
+        // one plane iteration; PH = i mod 3 selects the register slots at compile time; ts = i mod 3 is the ring slot of the
+        // TMA variant (= PH in the unrolled loop, a run-time value in the rotated one)
+        auto body = [&](auto ph, const int i, const int ts) {
             constexpr int PH = decltype(ph)::value;
             constexpr int CE = (PH + 2) % 3;               // centre plane slot
             constexpr int MI = (PH + 1) % 3;               // previous plane slot
             if constexpr (TMA) {
-                mbar_wait(&full[PH], (phases >> PH) & 1u);
-                phases ^= 1u << PH;
+                mbar_wait(&full[ts], (phases >> ts) & 1u);
+                phases ^= 1u << ts;
                 if constexpr (C::RESPF) cp_async_wait<0>();          // residual rows of the centre plane (issued one iteration ago)
             } else {
                 if (i + PD < niter) issue(i + PD);
@@ -537,7 +538,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
                 cp_async_wait<PD>();
             }
             {
-                const int sT = TMA ? PH : (i & (DT - 1));
+                const int sT = TMA ? ts : (i & (DT - 1));
                 float m = 0.f;
 #pragma unroll
                 for (int r = 0; r < RY; ++r) {
@@ -597,7 +598,7 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             __syncthreads();                               // exchange rows of iteration i-1 are visible
             if constexpr (TMA) {
                 // every thread has taken plane i-1 out of its slot (and is done with state plane i-6): refill them
-                if (tid == 0 && i + PD < niter) issue_tma(i + PD, (PH + PD) % DT);
+                if (tid == 0 && i + PD < niter) issue_tma(i + PD, ts + PD >= DT ? ts + PD - DT : ts + PD);
             }
             const int par_w = i & 1, par_r = par_w ^ 1;
             float4 out[RY];
@@ -802,14 +803,13 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             }
         };
 
-        // (the TMA variant indexes its ring by the iteration number mod 3 = the unrolled body: always unrolled)
-        if constexpr (TMA || (!CONS && !(HELDCOPY && S >= 3))) {
+        if constexpr (!CONS && !(HELDCOPY && S >= 3)) {
             for (int i = 0;;) {
-                body(IC<0>{}, i);
+                body(IC<0>{}, i, 0);
                 if (++i >= niter) break;
-                body(IC<1>{}, i);
+                body(IC<1>{}, i, 1);
                 if (++i >= niter) break;
-                body(IC<2>{}, i);
+                body(IC<2>{}, i, 2);
                 if (++i >= niter) break;
             }
         } else {
@@ -821,8 +821,10 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             // runs 786 GVox/s, rotated 806.  Without held-copy (no_instruction 0.47) and at two fused steps the unrolled
             // body wins (C4, S = 2: 728 vs 713), so those stay unrolled.
 #pragma unroll 1
+            int ts = 0;
             for (int i = 0; i < niter; ++i) {
-                body(IC<2>{}, i);                          // arrival in slot 2, centre 1, previous 0
+                body(IC<2>{}, i, ts);                      // arrival in slot 2, centre 1, previous 0
+                ts = ts == 2 ? 0 : ts + 1;
 #pragma unroll
                 for (int k = 0; k < S; ++k) {
 #pragma unroll
