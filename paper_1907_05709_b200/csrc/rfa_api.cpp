@@ -278,7 +278,7 @@ RfaTbPlan rfa_plan_blocked(int nx, int ny, int nz, int batch, int fused, const i
     const int S = fused;
     if (S < 1 || S > 4 || nx < 4 || (nx % 4) != 0 || ny < S || nz < S || batch < 1 || !resident_ctas) return best;
     // the kernel addresses one scenario with 32-bit float4 offsets; larger volumes take the plain kernel
-    if ((long long)(nx / 4) * ny * nz >= 0x7fffffffLL) return best;
+    if ((long long)(nx / 4) * ny * nz >= 0x7fffffffLL || (long long)nz * batch >= 0x7fffffffLL) return best;
     double best_cost = 1e300;
     for (int shape = 0; shape < RFA_N_SHAPES; ++shape) {
         double cost;

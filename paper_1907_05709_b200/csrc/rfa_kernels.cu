@@ -457,7 +457,9 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             if (gyf == 0) up_idx = tid;                      // outer faces: the voxel itself (R-7)
             if (gyf + RY == P.ny) dn_idx = NT + tid;
         }
-        const size_t base4 = (size_t)b * P.nz * plane4;
+        // (b * nz < 2^31 is checked by the planner: one 32 x 32 -> 64-bit multiply, cheap to recompute where the compiler
+        // prefers that to keeping five 64-bit pointers alive)
+        const size_t base4 = (size_t)((unsigned)b * (unsigned)P.nz) * plane4;
         const float4 *tin4 = reinterpret_cast<const float4 *>(P.tin) + base4;
         float4 *tout4 = reinterpret_cast<float4 *>(P.tout) + base4;
         const uint2 *rin2 = reinterpret_cast<const uint2 *>(P.rin) + base4;
