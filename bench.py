@@ -52,7 +52,7 @@ BYTES_BUILD = {"theta_read": 4.0, "theta_write": 4.0, "state_byte_read": 1.0, "r
 # held-copy / conduction): a run whose variant has no capture prints "traffic": null.
 NCU_TRAFFIC = {
     # variant: (bytes per launch, profile file)
-    "C4/S3/64x32/hc1/eq12": (587.2e6, "profiles/r2_blocked_s3_final_ncu.md"),
+    "C4/S3/64x32/hc1/eq12": (588.4e6, "profiles/r2_blocked_s3_final_ncu.md"),
     "C4/S3/64x32/hc0/eq12": (577.6e6, "profiles/r2_variants_ncu.md"),
     "C4/S2/64x32/hc1/eq12": (577.3e6, "profiles/r2_variants_ncu.md"),
     "C4/S1/128x16/hc1/eq12/tma": (569.1e6, "profiles/r2_variants_ncu.md"),
