@@ -693,7 +693,12 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
                                 const float4 c = q[k][CE][r];
                                 upk(add2(pk(c.x, c.y), zero2), o[r].x, o[r].y);
                                 upk(add2(pk(c.z, c.w), zero2), o[r].z, o[r].w);
-                                mx = max_abs4(o[r], mx);
+                            }
+                            // the copied rows are cold (|theta| < RFA_COMP_MIN, this branch) and stay what they are: their maximum
+                            // matters only to a necrosis threshold below RFA_COMP_MIN (T_a within 1 C of 60 C)
+                            if (thr_filter < RFA_COMP_MIN) {
+#pragma unroll
+                                for (int r = 0; r < RY; ++r) mx = max_abs4(o[r], mx);
                             }
                         } else {
                             load_rows();

@@ -282,7 +282,12 @@ __global__ void __launch_bounds__(32 * RFA_STREAM_NW, RFA_STREAM_MINB)
                                 const float4 c = q[CE][r];
                                 upk(add2(pk(c.x, c.y), zero2), o[r].x, o[r].y);
                                 upk(add2(pk(c.z, c.w), zero2), o[r].z, o[r].w);
-                                mx = max_abs4(o[r], mx);
+                            }
+                            // the copied rows are cold (|theta| < RFA_COMP_MIN, this branch) and stay what they are: their maximum
+                            // matters only to a necrosis threshold below RFA_COMP_MIN (T_a within 1 C of 60 C)
+                            if (thr_filter < RFA_COMP_MIN) {
+#pragma unroll
+                                for (int r = 0; r < RY; ++r) mx = max_abs4(o[r], mx);
                             }
                         } else {
 #pragma unroll

@@ -397,6 +397,25 @@ def test_held_copy_variant_is_bit_identical(rfa):
     assert float(ref[0].max()) == 90.0 and float(ref[0][11, 71, 110]) > 37.5
     for key, (T, N) in body.items():
         assert np.array_equal(T.view(np.uint32), ref[0].view(np.uint32)) and np.array_equal(N, ref[1]), key
+    # blood at 59.6 C: the necrosis threshold (0.4 C above T_a) lies BELOW the 1 C bound of the cold paths, so the copied rows'
+    # maxima matter to the necrosis filter (exterior held at 60.2 C: necrotic from the start; vessels at 59.6 C: not)
+    tab = W.tissue_table()
+    tab["t_init"][:] = 59.6
+    tab["t_init"][W.EXTERIOR] = 60.2
+    warm = {}
+    for kern, fused, hc in ((rfa.KERNEL_PLAIN, 1, 0), (rfa.KERNEL_BLOCKED, 3, 1), (rfa.KERNEL_BLOCKED, 2, 1), (rfa.KERNEL_BLOCKED, 1, 1)):
+        sim = rfa.RfaSim((nx, ny, nz), (0.9, 0.9, 1.2), lab, tab, 59.6, 0.05)
+        sim.configure(kern, fused)
+        if kern != rfa.KERNEL_PLAIN:
+            sim.configure_held_copy(hc)
+        sim.set_needle(0, mask, rfa.SRC_DIRICHLET, 90.0)
+        sim.step(20)
+        warm[(kern, fused)] = (sim.get_temperature(0), sim.get_necrosis(0))
+        sim.close()
+    ref = warm[(rfa.KERNEL_PLAIN, 1)]
+    assert ref[1][0, 0, 0] == 1 and 0 < int(ref[1].sum()) < ref[1].size
+    for key, (T, N) in warm.items():
+        assert np.array_equal(T.view(np.uint32), ref[0].view(np.uint32)) and np.array_equal(N, ref[1]), key
     sim = rfa.from_workload(W.c1_cube())                      # no held label at all: the plain variant is chosen
     assert sim.query_variant()["held_copy"] == 0
     sim.configure_held_copy(rfa.HELD_COPY_ON)
