@@ -65,3 +65,47 @@ def test_empty_rays_and_margin():
     tmax, depth, margin = RO.render_zone(T, (1, 1, 1), (0, 0, 1), (0, 1, 0), 12, 12, 1.0, 0.5, 42.5)
     assert tmax[0, 0] == 37.0 and depth[0, 0] == -1.0 and np.isinf(margin[0, 0])      # the ray misses the volume
     assert abs(tmax[6, 6] - 40.0) < 1e-12 and depth[6, 6] == -1.0 and abs(margin[6, 6] - 2.5) < 1e-12
+
+
+def test_linear_field_oblique_view_is_exact():
+    """Trilinear interpolation reproduces a linear field exactly, so for T = T0 + g . x the images of an OBLIQUE view have
+    closed forms to rounding: along a ray T is linear in the sample index m, tmax is its value at the last (or first)
+    sample inside the box of voxel centres, and the first sample with T >= iso solves one linear inequality.  The inside
+    range of m is computed here by testing every sample against the box (no slab formula shared with anything).
+    Catches swapped axes, wrong spacing, transposed weights and an off-by-half in the voxel-centre convention."""
+    nx, ny, nz = 14, 11, 9
+    h = np.array([0.7, 0.9, 1.3])
+    g = np.array([1.9, -0.8, 1.1])                          # deg C per mm
+    T0 = 40.0
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    T = T0 + g[0] * (i + 0.5) * h[0] + g[1] * (j + 0.5) * h[1] + g[2] * (k + 0.5) * h[2]
+    direction, up = np.array([1.0, 2.0, 3.0]), np.array([0.0, 1.0, 0.0])
+    W_, H_, pixel, step, iso = 9, 7, 0.75, 0.25, 52.0        # exactly representable in fp32 (the API takes floats)
+    tmax, depth, _ = RO.render_zone(T, tuple(h), tuple(direction), tuple(up), W_, H_, pixel, step, iso)
+    w = direction / np.linalg.norm(direction)
+    e1 = np.cross(up, w)
+    e1 /= np.linalg.norm(e1)
+    e2 = np.cross(w, e1)
+    n = np.array([nx, ny, nz], dtype=np.float64)
+    c, R = 0.5 * n * h, 0.5 * np.sqrt(np.sum((n * h) ** 2))
+    ns = int(np.floor(2.0 * R / step)) + 1
+    m = np.arange(ns)
+    seen_inside = 0
+    for py in range(H_):
+        for px in range(W_):
+            o = c + (px - 0.5 * (W_ - 1)) * pixel * e1 + (py - 0.5 * (H_ - 1)) * pixel * e2 - R * w
+            p = o[None, :] + (m * step)[:, None] * w[None, :]          # sample positions in mm
+            q = p / h - 0.5
+            inside = np.all((q >= 0.0) & (q <= n - 1.0), axis=1)
+            if not inside.any():
+                assert tmax[py, px] == 37.0 and depth[py, px] == -1.0
+                continue
+            seen_inside += 1
+            Tm = T0 + p[inside] @ g                                  # the field itself at the samples that count
+            assert abs(tmax[py, px] - Tm.max()) < 1e-9
+            hit = np.nonzero(Tm >= iso)[0]
+            if hit.size:
+                assert depth[py, px] == m[inside][hit[0]] * step
+            else:
+                assert depth[py, px] == -1.0
+    assert seen_inside > 20
