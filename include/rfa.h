@@ -211,6 +211,34 @@ int rfa_set_probes(rfa_sim *s, int n_probes, const int64_t *index);
  * the records have arrived in `out`. */
 int rfa_step_record(rfa_sim *s, int n, int every, float *out);
 
+/* rfa_step_record for callers that cannot allocate device memory when they call it.
+ *
+ * Why it exists: rfa_set_probes and rfa_step_record (host `out`) get the probe list and the row buffer from cudaMalloc, on
+ * the first use and again whenever a longer series is asked for.  cudaMalloc / cudaFree wait for the whole GPU, so inside a
+ * running frame loop (Alg. 2) they stall every stream of the device; and a host application that has handed the card's
+ * memory to its own pool at start-up, or runs under a fixed memory budget, gets an error from them.  This call uses neither:
+ * list and rows live in a fixed array inside the library image, RFA_STATIC_RECORD_MAX_PROBES * 8 +
+ * RFA_STATIC_RECORD_MAX_FLOATS * 4 bytes (1 MiB + 8 KiB), which every GPU that loads librfa.so holds until the process ends.
+ * It calls no cudaMalloc, cudaFree or other allocating routine.  (rfa_create allocates nothing on the device either when it
+ * is given a workspace.)
+ *
+ *   n, every   as rfa_step_record: n time steps, one record after every `every` of them (n a multiple of every)
+ *   n_probes   1 .. RFA_STATIC_RECORD_MAX_PROBES
+ *   index      host, n_probes flat voxel indices (as rfa_set_probes); read before the call returns.  The list given to
+ *              rfa_set_probes is neither used nor changed.
+ *   out        host or device, (n/every)*n_probes floats, out[m*n_probes + p] = T (deg C) at probe p after (m+1)*every steps
+ * Limits: n_probes > RFA_STATIC_RECORD_MAX_PROBES or (n/every)*n_probes > RFA_STATIC_RECORD_MAX_FLOATS -> RFA_E_INVALID
+ * with both numbers in rfa_last_error(), nothing stepped; record a longer run as several calls.
+ * Same kernels and same arithmetic as rfa_step_record: equal inputs give equal bits.  Returns after the records have arrived.
+ *
+ * Sharing: there is ONE such array per GPU for the whole process.  It keeps the previous call's contents (harmless: a call
+ * overwrites every element it later reads, nothing has to start at zero), and two calls that run on the same GPU at the same
+ * time -- from two host threads, on any simulations -- overwrite each other's rows.  The library takes no lock: serialise them.
+ * First use: the first call on a GPU asks the CUDA runtime for the array's device address (once per device, kept afterwards).
+ * Make that first call at start-up, before any stream capture is begun. */
+enum { RFA_STATIC_RECORD_MAX_PROBES = 1024, RFA_STATIC_RECORD_MAX_FLOATS = 262144 };
+int rfa_step_record_static(rfa_sim *s, int n, int every, int n_probes, const int64_t *index, float *out);
+
 /* Frame hand-off (Alg. 2): device pointer of the finished image of one scenario as stored,
  * theta = T - t_blood (fp32, nx*ny*nz, x fastest), and t_blood.  The image stays untouched by the NEXT
  * launch of this simulation (it writes the other buffer) and is overwritten by the one after it: a

@@ -24,12 +24,13 @@ COND_EQ12, COND_FACE = 0, 1
 HELD_COPY_AUTO, HELD_COPY_OFF, HELD_COPY_ON = -1, 0, 1
 STAGING_AUTO, STAGING_CP_ASYNC, STAGING_TMA = -1, 0, 1
 RES_PREFETCH_AUTO, RES_PREFETCH_OFF, RES_PREFETCH_ON = -1, 0, 1
+STATIC_RECORD_MAX_PROBES, STATIC_RECORD_MAX_FLOATS = 1024, 262144   # rfa_step_record_static (include/rfa.h)
 
 # every symbol include/rfa.h declares
 EXPORTS = [
     "rfa_workspace_bytes", "rfa_stability_number", "rfa_create", "rfa_set_needle", "rfa_set_temperature",
     "rfa_step", "rfa_get_temperature", "rfa_get_necrosis", "rfa_necrotic_voxels", "rfa_configure",
-    "rfa_set_conduction", "rfa_query", "rfa_query_variant", "rfa_configure_held_copy", "rfa_configure_staging", "rfa_configure_tile", "rfa_configure_residual_prefetch", "rfa_query_hot_fraction", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_current_frame",
+    "rfa_set_conduction", "rfa_query", "rfa_query_variant", "rfa_configure_held_copy", "rfa_configure_staging", "rfa_configure_tile", "rfa_configure_residual_prefetch", "rfa_query_hot_fraction", "rfa_plan_query", "rfa_set_probes", "rfa_step_record", "rfa_step_record_static", "rfa_current_frame",
     "rfa_warp_temperature", "rfa_render_zone",
     "rfa_synchronize", "rfa_destroy", "rfa_last_error",
 ]
@@ -112,6 +113,8 @@ def load_library() -> ctypes.CDLL:
     lib.rfa_set_probes.restype = ctypes.c_int
     lib.rfa_step_record.argtypes = [vp, ctypes.c_int, ctypes.c_int, vp]
     lib.rfa_step_record.restype = ctypes.c_int
+    lib.rfa_step_record_static.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int64), vp]
+    lib.rfa_step_record_static.restype = ctypes.c_int
     lib.rfa_current_frame.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.POINTER(ctypes.c_float)]
     lib.rfa_current_frame.restype = ctypes.c_int
     lib.rfa_warp_temperature.argtypes = [vp, ctypes.c_int, vp, ctypes.c_float, vp]
@@ -292,6 +295,21 @@ class RfaSim:
         if out is None:
             out = np.empty((rows, getattr(self, "n_probes", 0)), dtype=np.float32)
         _check(self._lib.rfa_step_record(self._handle, int(n), int(every), _ptr(out)))
+        return out
+
+    def step_record_static(self, n: int, every: int, index, out=None):
+        """``step_record`` for callers that must not allocate device memory at this point (a running frame loop, which a
+        cudaMalloc would stall; an application whose memory pool owns the whole card): the probe list ``index`` is passed
+        here instead of to ``set_probes``, and list and rows go through a fixed 1 MiB array inside librfa.so, so at most
+        ``STATIC_RECORD_MAX_PROBES`` probes and ``STATIC_RECORD_MAX_FLOATS`` recorded values per call.  One array per GPU:
+        do not run two of these calls on one GPU at the same time.  Same bits as ``step_record``."""
+        idx = np.ascontiguousarray(index, dtype=np.int64).reshape(-1)
+        rows = int(n) // max(int(every), 1)
+        if out is None:
+            out = np.empty((rows, int(idx.size)), dtype=np.float32)
+        _check(self._lib.rfa_step_record_static(self._handle, int(n), int(every), int(idx.size),
+                                                idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)) if idx.size else None,
+                                                _ptr(out)))
         return out
 
     def current_frame(self, scenario: int = 0):

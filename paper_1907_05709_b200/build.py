@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librfa.so")
-SOURCES = ["rfa_kernels.cu", "rfa_stream.cu", "rfa_view.cu", "rfa_api.cpp"]
+SOURCES = ["rfa_kernels.cu", "rfa_stream.cu", "rfa_view.cu", "rfa_noalloc.cu", "rfa_api.cpp"]
 HEADERS = ["rfa_device.cuh", "rfa_packed.cuh", "rfa_internal.h", os.path.join("..", "..", "include", "rfa.h")]
 
 NVCC_FLAGS = [

@@ -1008,6 +1008,44 @@ extern "C" int rfa_step_record(rfa_sim *s, int n, int every, float *out)
     return RFA_OK;
 }
 
+// rfa_step_record without any allocation: probe list and rows in the per-GPU static array of rfa_noalloc.cu (include/rfa.h
+// says for whom).  No cudaMalloc / cudaFree / cudaMallocHost here or below: advance() only launches, the three
+// rfa_static_record_* helpers only copy and launch.
+extern "C" int rfa_step_record_static(rfa_sim *s, int n, int every, int n_probes, const int64_t *index, float *out)
+{
+    if (!s) return fail(RFA_E_INVALID, "null simulation handle");
+    DeviceGuard dg(s);
+    if (n < 0 || every < 1 || (n % every) != 0) return fail(RFA_E_INVALID, "n must be a non-negative multiple of every >= 1");
+    if (n_probes < 1 || !index) return fail(RFA_E_INVALID, "need at least one probe and its index list");
+    if (!out) return fail(RFA_E_INVALID, "out is null");
+    if (n_probes > RFA_STATIC_RECORD_MAX_PROBES)
+        return fail(RFA_E_INVALID, "%d probes: the static scratch holds at most %d (RFA_STATIC_RECORD_MAX_PROBES); use rfa_set_probes + rfa_step_record",
+                    n_probes, (int)RFA_STATIC_RECORD_MAX_PROBES);
+    const size_t rows = (size_t)(n / every), need = rows * (size_t)n_probes;
+    if (need > (size_t)RFA_STATIC_RECORD_MAX_FLOATS)
+        return fail(RFA_E_INVALID, "%zu records x %d probes = %zu floats: the static scratch holds at most %d (RFA_STATIC_RECORD_MAX_FLOATS); "
+                    "record the run as several shorter calls", rows, n_probes, need, (int)RFA_STATIC_RECORD_MAX_FLOATS);
+    const long long total = (long long)s->nvox * s->g.batch;
+    for (int p = 0; p < n_probes; ++p)
+        if (index[p] < 0 || index[p] >= total) return fail(RFA_E_INVALID, "probe %d: index %lld outside [0,%lld)", p, (long long)index[p], total);
+    if (rows == 0) return RFA_OK;
+    static_assert(sizeof(long long) == sizeof(int64_t), "probe indices are 64-bit");
+    cudaError_t e = rfa_static_record_begin(n_probes, (const long long *)index, s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "static scratch set-up / probe upload");
+    for (size_t m = 0; m < rows; ++m) {
+        int rc = advance(s, every);
+        if (rc) return rc;
+        e = rfa_static_record_probe(s->g, n_probes, s->theta[s->cur], m, s->stream);
+        s->launches++;
+        if (e != cudaSuccess) return cuda_fail(e, "probe kernel (static scratch)");
+    }
+    e = rfa_static_record_fetch(out, need, s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "record download (static scratch)");
+    e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "step_record_static");
+    return RFA_OK;
+}
+
 extern "C" int rfa_current_frame(rfa_sim *s, int scenario, const float **theta_dev, float *t_blood_c)
 {
     int rc = check_sim(s, scenario);

@@ -106,6 +106,12 @@ cudaError_t rfa_launch_render(const RfaGrid &g, int scenario, const RfaRay &ray,
                               float iso_theta, float *tmax_dev, float *depth_dev /*may be null*/, cudaStream_t st);
 cudaError_t rfa_launch_probe(const RfaGrid &g, int n, const long long *index_dev, const float *theta /*all scenarios*/,
                              float *out_dev, cudaStream_t st);
+// ---- rfa_step_record_static: probe list and rows in a file-scope device array (rfa_noalloc.cu), no allocation anywhere ----
+// begin: probe list (host) -> head of the array;  probe: the probe kernel into row `row`;  fetch: rows -> out (host or device).
+// All asynchronous on `st`, all for the CURRENT device (the first of them on a device looks the array's address up).
+cudaError_t rfa_static_record_begin(int n_probes, const long long *index_host, cudaStream_t st);
+cudaError_t rfa_static_record_probe(const RfaGrid &g, int n_probes, const float *theta /*all scenarios*/, size_t row, cudaStream_t st);
+cudaError_t rfa_static_record_fetch(float *out, size_t floats, cudaStream_t st);
 cudaError_t rfa_launch_count(const RfaGrid &g, int scenario, const uint8_t *state, uint32_t label_held_mask,
                              unsigned long long *counters_dev /*2*/, cudaStream_t st);
 // kap: null = Eq. 12 as printed; else device table [16][16] of Kf/K_c - 1 (conservative conduction, R-28)

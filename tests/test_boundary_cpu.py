@@ -92,6 +92,7 @@ def test_null_handles_are_rejected(lib):
     for fn in (lib.rfa_configure_held_copy, lib.rfa_configure_staging, lib.rfa_configure_tile, lib.rfa_configure_residual_prefetch):
         assert fn(None, 0) == binding.RFA_E_INVALID
     assert lib.rfa_query_hot_fraction(None, None, None) == binding.RFA_E_INVALID
+    assert lib.rfa_step_record_static(None, 1, 1, 0, None, None) == binding.RFA_E_INVALID
     lib.rfa_destroy(None)
 
 
