@@ -458,6 +458,81 @@ def test_probe_series_monotone_symmetric_affine(oracle):
     assert s90.max() < 90.0 and s90.min() >= 37.0
 
 
+@pytest.mark.parametrize("every", [1, 4])
+def test_probe_series_row_m_is_the_field_after_m_plus_1_times_every_steps(oracle, every):
+    """Pin of OracleSim.step_record's row <-> step mapping on the paper's probe set-up (Fig. 6 :250,
+    Fig. 14 :282): row m must equal the field of a FRESH simulation advanced (m+1)*every times by plain step(1) calls and
+    read at the probe voxels.  A record taken before the step, a row shifted by one record, or `every` applied once too
+    often or too seldom all change some row: the probes heat strictly monotonically, so consecutive fields differ."""
+    w = W.paper_probe_case(90.0, n=32, steps=24)
+    pr = W.fig6_probes(w.dims, w.spacing_mm, w.meta["centre_voxel"]).ravel()
+    nd = w.needles[0]
+
+    def fresh():
+        sim = oracle.OracleSim(w.dims, w.spacing_mm, w.labels, w.table, w.t_blood, w.dt)
+        sim.set_needle(nd.mask, nd.mode, nd.value)
+        return sim
+
+    rec = fresh().step_record(w.steps, every, pr)
+    assert rec.shape == (w.steps // every, pr.size)
+    nx, ny, nz = w.dims
+    ref = fresh()
+    fields = []                                   # fields[t] = probe values after t+1 single steps, read by (k, j, i)
+    for _ in range(w.steps):
+        ref.step(1)
+        fields.append(np.array([ref.T[p // (nx * ny), (p // nx) % ny, p % nx] for p in pr]))
+    for m in range(rec.shape[0]):
+        assert np.array_equal(rec[m], fields[(m + 1) * every - 1]), f"row {m} is not the field after {(m + 1) * every} steps"
+    # the pin has teeth: neighbouring candidates (one step / one record earlier or later) are different fields
+    assert not np.array_equal(fields[every - 1], fields[every]) and not np.array_equal(fields[0], np.full(pr.size, 37.0))
+    if every > 1:
+        assert not np.array_equal(rec[0], fields[0])
+    # the simulation that recorded has advanced n steps in total
+    sim = fresh()
+    sim.step_record(w.steps, every, pr)
+    assert sim.steps_done == w.steps and np.array_equal(sim.T, ref.T)
+
+
+def test_necrotic_volume_counts_tissue_voxels_in_cubic_millimetres(oracle):
+    """Pin of OracleSim.necrotic_volume_mm3 (necrosis at T >= 60 C: PAPER.md:37; reported volume without needle and
+    held-label voxels: DESIGN.md R-13) on a hand-built anisotropic grid, 0.7 x 0.9 x 1.3 mm, where every count is known
+    by construction: no step is taken, the mask comes from the initial image alone."""
+    dims, spacing = (6, 5, 4), (0.7, 0.9, 1.3)
+    vox = 0.7 * 0.9 * 1.3                                             # mm^3, typed here from the spacing
+    table = W.make_table([
+        (0.52, 1079.0, 3540.0, 0.0, 0.0, 37.0, 0),                   # 0 tissue, cold
+        (0.52, 1079.0, 3540.0, 0.0, 0.0, 61.0, 0),                   # 1 tissue that starts above the threshold
+        (0.512, 1060.0, 3600.0, 0.0, 0.0, 75.0, W.TISSUE_HELD),       # 2 HELD label that is hot (not tissue damage)
+        (0.52, 1079.0, 3540.0, 0.0, 0.0, 59.999, 0),                 # 3 tissue just below the threshold
+        (0.52, 1079.0, 3540.0, 0.0, 0.0, 60.0, 0),                   # 4 tissue exactly at it: inclusive
+    ])
+    lab = np.zeros((4, 5, 6), np.uint8)                               # (nz, ny, nx)
+    lab[0, 0, 0:5] = 1                                                # 5 hot tissue voxels
+    lab[1, 1:4, 2] = 2                                                # 3 hot held-label voxels
+    lab[2, 4, 0:2] = 3                                                # 2 voxels at 59.999: not necrotic
+    lab[3, 2, 1:5] = 4                                                # 4 voxels at exactly 60.0: necrotic
+    sim = oracle.OracleSim(dims, spacing, lab, table, 37.0, 0.05)
+    assert int(sim.necro.sum()) == 5 + 3 + 4
+    assert sim.necrotic_volume_mm3() == pytest.approx((5 + 4) * vox, rel=1e-12)
+    assert sim.necrotic_volume_mm3(exclude_held=False) == pytest.approx((5 + 3 + 4) * vox, rel=1e-12)
+    # a Dirichlet needle at 90 C over 7 voxels: 2 of them were hot tissue already, 1 is a held-label voxel, 4 were cold
+    mask = np.zeros_like(lab)
+    mask[0, 0, 3:5] = 1
+    mask[1, 1, 2] = 1
+    mask[2, 0:4, 5] = 1
+    sim.set_needle(mask, W.SRC_DIRICHLET, 90.0)
+    assert int(sim.necro.sum()) == 12 + 4
+    assert sim.necrotic_volume_mm3() == pytest.approx((3 + 4) * vox, rel=1e-12)              # tissue only: 5 - 2 + 4
+    assert sim.necrotic_volume_mm3(exclude_held=False) == pytest.approx(16 * vox, rel=1e-12)
+    # a POWER needle heats but holds nothing, yet its voxels are electrode, not tissue (R-13): a hot tissue voxel under
+    # the mask leaves the reported volume; the 4 voxels the Dirichlet needle burnt stay in the sticky mask and count again
+    mask2 = np.zeros_like(lab)
+    mask2[3, 2, 1] = 1
+    sim.set_needle(mask2, W.SRC_POWER, 1.0e6)
+    assert sim.necrotic_volume_mm3(exclude_held=False) == pytest.approx(16 * vox, rel=1e-12)
+    assert sim.necrotic_volume_mm3() == pytest.approx((5 + 3 + 4) * vox, rel=1e-12)          # 5 hot + (4 - 1) at 60 + 4 burnt
+
+
 # ----------------------------------------------------------------------------------------------
 # Row f1: conservative heterogeneous conduction div(K grad T) of Eq. 9 (PAPER.md:102), harmonic-mean
 # face conductivities (DESIGN.md R-28).  Pins of rfa_oracle_step_cons.
