@@ -827,8 +827,8 @@ __global__ void __launch_bounds__(TX *TY, MINB) rfa_blocked_kernel(const __grid_
             // paths side by side (copy / bracket): unrolled, no_instruction is its largest stall (1.36 per issue) and C4
             // runs 786 GVox/s, rotated 806.  Without held-copy (no_instruction 0.47) and at two fused steps the unrolled
             // body wins (C4, S = 2: 728 vs 713), so those stay unrolled.
-#pragma unroll 1
             int ts = 0;
+#pragma unroll 1
             for (int i = 0; i < niter; ++i) {
                 body(IC<2>{}, i, ts);                      // arrival in slot 2, centre 1, previous 0
                 ts = ts == 2 ? 0 : ts + 1;
