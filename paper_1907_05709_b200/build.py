@@ -12,7 +12,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librfa.so")
 SOURCES = ["rfa_kernels.cu", "rfa_stream.cu", "rfa_view.cu", "rfa_noalloc.cu", "rfa_api.cpp"]
-HEADERS = ["rfa_device.cuh", "rfa_packed.cuh", "rfa_internal.h", os.path.join("..", "..", "include", "rfa.h")]
+# every header under csrc/ (rfa_tma.cuh included: an edit of the mbarrier / TMA wrappers must rebuild the kernels) + the C ABI
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))) + [os.path.join("..", "..", "include", "rfa.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
