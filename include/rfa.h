@@ -170,7 +170,9 @@ int rfa_configure_held_copy(rfa_sim *s, int mode);
  * of Alg. 1): per-thread cp.async, or one bulk tensor copy (Tensor Memory Accelerator) per tile plane issued by
  * a single thread.  The TMA variant exists for 2 and 3 fused steps in RFA_COND_EQ12 mode on grids with nx % 16 == 0 and ny
  * even; AUTO (the default) takes it where it measured faster (the 128 x 16 tile).  All settings give bit-identical fields.  Returns RFA_E_INVALID,
- * leaving the setting unchanged, when RFA_STAGING_TMA is asked for a grid that has no such variant. */
+ * leaving the setting unchanged, when RFA_STAGING_TMA is asked for a grid that has no such variant.  The setting is kept across
+ * rfa_set_conduction: while RFA_COND_FACE is active it has no effect (that mode has cp.async variants only; rfa_query_variant
+ * shows the staging that really runs). */
 enum { RFA_STAGING_AUTO = -1, RFA_STAGING_CP_ASYNC = 0, RFA_STAGING_TMA = 1 };
 int rfa_configure_staging(rfa_sim *s, int mode);
 
@@ -187,7 +189,8 @@ int rfa_query_hot_fraction(rfa_sim *s, double *fraction, int *prefetch_on);
 
 /* Force the tile shape of the blocked kernel: 0 = 64 x 32 voxels (16 x 16 threads), 1 = 128 x 16 (32 x 8 threads), -1 = the
  * planner's choice (the default).  For A/B measurements; all shapes give bit-identical fields.  RFA_E_INVALID, leaving the
- * setting unchanged, if the shape cannot run the configured number of fused steps on this grid. */
+ * setting unchanged, if the shape cannot run the configured number of fused steps on this grid in the active conduction mode
+ * (checked for every kernel setting except RFA_KERNEL_PLAIN, which has no tiles). */
 int rfa_configure_tile(rfa_sim *s, int shape);
 
 /* Host-only view of the blocked kernel's launch plan for a grid (no GPU needed; used by the unit tests

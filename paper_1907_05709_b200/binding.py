@@ -173,6 +173,23 @@ def _ptr(x):
     return ctypes.c_void_p(x.data_ptr())
 
 
+def _check_out(x, n_elem: int, what: str, np_dtype=np.float32):
+    """An output buffer handed to the library by raw address: it must hold >= n_elem contiguous elements of the
+    right type, or the library would write past its end (host) / fault (device)."""
+    if isinstance(x, np.ndarray):
+        ok = x.dtype == np_dtype and x.flags["C_CONTIGUOUS"] and x.flags["WRITEABLE"]
+        size = x.size
+    else:
+        import torch
+        want = {np.float32: torch.float32, np.uint8: torch.uint8}[np_dtype]
+        ok = x.dtype == want and x.is_contiguous()
+        size = x.numel()
+    if not ok:
+        raise ValueError(f"{what}: need a contiguous {np.dtype(np_dtype).name} buffer")
+    if size < n_elem:
+        raise ValueError(f"{what}: buffer of {size} elements, need {n_elem}")
+
+
 class RfaSim:
     """One simulation: ``batch`` scenarios sharing a label volume.  Mirrors include/rfa.h one to one."""
 
@@ -235,6 +252,7 @@ class RfaSim:
         nx, ny, nz = self.dims
         if out is None:
             out = np.empty((nz, ny, nx), dtype=np.float32)
+        _check_out(out, nx * ny * nz, "get_temperature out", np.float32)
         _check(self._lib.rfa_get_temperature(self._handle, int(scenario), _ptr(out)))
         return out
 
@@ -242,6 +260,7 @@ class RfaSim:
         nx, ny, nz = self.dims
         if out is None:
             out = np.empty((nz, ny, nx), dtype=np.uint8)
+        _check_out(out, nx * ny * nz, "get_necrosis out", np.uint8)
         _check(self._lib.rfa_get_necrosis(self._handle, int(scenario), _ptr(out)))
         return out
 
@@ -294,6 +313,7 @@ class RfaSim:
         rows = int(n) // max(int(every), 1)
         if out is None:
             out = np.empty((rows, getattr(self, "n_probes", 0)), dtype=np.float32)
+        _check_out(out, rows * getattr(self, "n_probes", 0), "step_record out")
         _check(self._lib.rfa_step_record(self._handle, int(n), int(every), _ptr(out)))
         return out
 
@@ -307,6 +327,7 @@ class RfaSim:
         rows = int(n) // max(int(every), 1)
         if out is None:
             out = np.empty((rows, int(idx.size)), dtype=np.float32)
+        _check_out(out, rows * int(idx.size), "step_record_static out")
         _check(self._lib.rfa_step_record_static(self._handle, int(n), int(every), int(idx.size),
                                                 idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)) if idx.size else None,
                                                 _ptr(out)))
@@ -324,6 +345,7 @@ class RfaSim:
         d = disp if not isinstance(disp, np.ndarray) else np.ascontiguousarray(disp, dtype=np.float32)
         if out is None:
             out = np.empty((nz, ny, nx), dtype=np.float32)
+        _check_out(out, nx * ny * nz, "warp_temperature out")
         _check(self._lib.rfa_warp_temperature(self._handle, int(scenario), _ptr(d), float(scale), _ptr(out)))
         return out
 
@@ -337,6 +359,9 @@ class RfaSim:
             tmax = np.empty((height, width), dtype=np.float32)
         if depth is None and want_depth:
             depth = np.empty((height, width), dtype=np.float32)
+        _check_out(tmax, int(width) * int(height), "render_zone tmax")
+        if depth is not None:
+            _check_out(depth, int(width) * int(height), "render_zone depth")
         _check(self._lib.rfa_render_zone(self._handle, int(scenario), ctypes.byref(v), _ptr(tmax),
                                          _ptr(depth) if depth is not None else None))
         return tmax, depth

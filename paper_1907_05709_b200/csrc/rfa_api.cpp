@@ -792,7 +792,9 @@ extern "C" int rfa_configure_tile(rfa_sim *s, int shape)
     const int old = s->force_shape;
     s->force_shape = shape;
     make_plans(s);
-    if (s->kernel == RFA_KERNEL_BLOCKED && !s->plans()[s->fused].ok) {
+    // a forced shape that cannot run is refused whatever the kernel setting: under RFA_KERNEL_AUTO it would otherwise
+    // drop to the plain kernel without a word (only RFA_KERNEL_PLAIN, which has no tiles, takes any shape)
+    if (shape != -1 && s->kernel != RFA_KERNEL_PLAIN && !s->plans()[s->fused].ok) {
         s->force_shape = old;
         make_plans(s);
         return fail(RFA_E_INVALID, "tile shape %d cannot run the configured %d fused steps on this grid", shape, s->fused);
@@ -897,7 +899,9 @@ static int advance(rfa_sim *s, int n)
         {
             e = rfa_launch_stream(s->g, s->stream_plan, s->tm_theta[s->cur], s->tm_state, tout, rin, rout, s->state, s->tables,
                                   s->counters + 4, s->stream_draws, s->stream);
-            s->stream_draws += (unsigned long long)s->stream_plan.n_items;   // every launch draws exactly n_items times
+            // every launch that ran draws exactly n_items times; one that was never queued drew nothing, and counting it
+            // would hand every later launch a work_base ahead of the device counter (items skipped or done twice)
+            if (e == cudaSuccess) s->stream_draws += (unsigned long long)s->stream_plan.n_items;
         }
         else if (k == RFA_KERNEL_BLOCKED) {
             const RfaTbPlan &pl = s->plans()[did];

@@ -692,6 +692,29 @@ def test_boundary_validation_on_a_live_simulation(rfa):
             sim.step(3)
             T1 = sim.get_temperature(0)
         assert not np.array_equal(T0, T1)
+    # output buffers are checked by the binding before their raw address reaches the library
+    with pytest.raises(ValueError):
+        sim.get_temperature(0, out=np.empty(w.n_voxels - 1, np.float32))
+    with pytest.raises(ValueError):
+        sim.get_temperature(0, out=np.empty(w.n_voxels, np.float64))
+    with pytest.raises(ValueError):
+        sim.render_zone(0, (0, 0, 1), (0, 1, 0), 16, 16, 1.0, 1.0, tmax=np.empty((16, 32), np.float32)[:, ::2])
+    with pytest.raises(ValueError):
+        sim.render_zone(0, (0, 0, 1), (0, 1, 0), 16, 16, 1.0, 1.0, depth=torch.empty(255, dtype=torch.float32, device="cuda"))
+    sim.set_probes([0, 1, 2])
+    with pytest.raises(ValueError):
+        sim.step_record(4, 2, out=np.empty((2, 2), np.float32))
+    sim.close()
+    # a forced tile shape that cannot run is refused under every kernel setting but PLAIN (nx % 4 != 0: no blocked plan)
+    sim = rfa.from_workload(W.ragged_phantom(dims=(45, 38, 29), spacing=(0.7, 0.9, 1.3), steps=3))
+    for shape in (0, 1):
+        with pytest.raises(rfa.RfaError) as ei:
+            sim.configure_tile(shape)
+        assert ei.value.code == rfa.RFA_E_INVALID
+    sim.configure_tile(-1)
+    sim.configure(rfa.KERNEL_PLAIN, 0)
+    sim.configure_tile(1)
+    sim.step(3)
     sim.close()
 
 
