@@ -47,23 +47,32 @@ METRIC = "GVoxel-updates/s"
 # measured DRAM traffic is 8.5-8.8 B per voxel per launch, the `traffic` key).
 BYTES_SURVEY = {"theta_read": 4.0, "theta_write": 4.0, "label_byte": 1.0, "necrosis_byte": 1.0}
 BYTES_BUILD = {"theta_read": 4.0, "theta_write": 4.0, "state_byte_read": 1.0, "residual_fp16_write": 2.0}
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel, from the `ncu --set full`
-# captures summarised under profiles/.  Keyed by the variant string of the run (workload / fused steps / tile /
-# held-copy / conduction): a run whose variant has no capture prints "traffic": null.
-NCU_TRAFFIC = {
-    # variant: (bytes per launch, profile file)
-    "C4/S3/64x32/hc1/eq12": (588.4e6, "profiles/r2_blocked_s3_final_ncu.md"),
-    "C4/S3/64x32/hc0/eq12": (577.6e6, "profiles/r2_variants_ncu.md"),
-    "C4/S2/64x32/hc1/eq12": (577.3e6, "profiles/r2_variants_ncu.md"),
-    "C4/S1/128x16/hc1/eq12/tma": (569.1e6, "profiles/r2_variants_ncu.md"),
-    "C4/S1/128x16/hc0/eq12/tma": (569.1e6, "profiles/r2_variants_ncu.md"),
-    "C3/S3/64x32/hc0/eq12/rpf": (120.6e6, "profiles/r2_blocked_ab_ncu.md"),
-    "C3/S3/64x32/hc0/eq12": (120.6e6, "profiles/r2_blocked_ab_ncu.md"),
-    "C5/S2/128x16/hc0/eq12/tma": (1200.1e6, "profiles/r2_blocked_ab_ncu.md"),
-    "C4/S3/64x32/hc1/face": (641.8e6, "profiles/r2_variants_ncu.md"),
-    "C4F/S3/64x32/hc1/face/rpf": (870.9e6, "profiles/r2_blocked_ab_ncu.md"),
-    "C4/plain": (840.3e6, "profiles/r2_variants_ncu.md"),
+# Per launch of the dominant kernel, from the ncu rows summarised under profiles/: DRAM bytes (dram__bytes_read.sum +
+# dram__bytes_write.sum) and warp instructions executed (smsp__inst_executed.sum).  Keyed by the variant string of the run
+# (workload / fused steps / tile / held-copy / conduction / staging / residual prefetch): a run whose variant has no row
+# prints "traffic": null and "issue": null.
+_V = "profiles/r2_variants_final_ncu.md"
+_AB = "profiles/r2_blocked_ab_ncu.md"
+NCU_ROWS = {
+    # variant: (DRAM bytes per launch, warp instructions per launch or None, profile file)
+    "C4/S3/64x32/hc1/eq12": (588.4e6, 147.27e6, "profiles/r2_blocked_s3_final_ncu.md"),
+    "C4/S3/64x32/hc0/eq12": (577.4e6, 164.02e6, _V),
+    "C4/S3/64x32/hc1/eq12/tma": (592.5e6, 154.73e6, _V),
+    "C4/S2/64x32/hc1/eq12": (577.5e6, 89.80e6, _V),
+    "C4/S4/64x32/hc1/eq12": (580.2e6, 198.97e6, _V),
+    "C4/S1/64x32/hc1/eq12": (578.0e6, 47.44e6, _V),
+    "C4/S1/128x16/hc1/eq12/tma": (568.9e6, 50.86e6, _V),
+    "C4/S1/128x16/hc0/eq12/tma": (569.3e6, 57.81e6, _V),
+    "C3/S3/64x32/hc0/eq12/rpf": (120.6e6, None, _AB),
+    "C3/S3/64x32/hc0/eq12": (119.0e6, 46.51e6, _V),
+    "C5/S2/128x16/hc0/eq12/tma": (1200.2e6, 220.86e6, _V),
+    "C5/S3/128x16/hc0/eq12/tma": (1185.6e6, 367.36e6, _V),
+    "C4/S3/64x32/hc1/face": (642.4e6, 182.25e6, _V),
+    "C4F/S3/64x32/hc1/face": (855.0e6, 345.18e6, _V),
+    "C4F/S3/64x32/hc1/face/rpf": (870.9e6, None, _AB),
+    "C4/plain": (840.6e6, 494.93e6, _V),
 }
+NCU_TRAFFIC = {k: (v[0], v[2]) for k, v in NCU_ROWS.items()}
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
 
@@ -335,17 +344,47 @@ def run_ours(args):
     launch_us = ms_main * 1e3 / max(n_main, 1) if n_main else ms_local * 1e3 / max(launches, 1)
     b_survey = sum(BYTES_SURVEY.values()) * nvox_all
     b_build = sum(BYTES_BUILD.values()) * nvox_all
-    achieved = b_survey / (launch_us * 1e-6) / 1e9
+    # Bytes the launch really moves.  Where an ncu capture of this variant exists: its DRAM traffic.  Otherwise this
+    # build's own count: 4 B theta read + 4 B theta write + 1 B state byte (label, flags and the necrosis bit share it;
+    # it is written back only where it changes), plus the fp16 residual (2 B read + 2 B written) for the share of rows
+    # that are hot, which the kernels count themselves (rfa_query_hot_fraction).  SURVEY.md 8(d)'s 10 B per voxel has a
+    # separate necrosis byte that this build does not move: kept as frac_survey_10B, not as the headline fraction.
     vkey = (variant_key(w.name, variant) + ("/tma" if variant.get("staging") == binding.STAGING_TMA else "") +
             ("/rpf" if variant.get("residual_prefetch") else "")) if (blocked or stream_k) else f"{w.name}/plain"
     traffic, traffic_src = NCU_TRAFFIC.get(vkey, (None, None))
+    hot = float(variant.get("hot_fraction", 0.0) or 0.0) if (blocked or stream_k) else 1.0
+    bytes_counted = {"theta_read": 4.0, "theta_write": 4.0, "state_byte_read": 1.0, "residual_fp16_read_write_hot_rows": 4.0 * hot}
+    b_counted = sum(bytes_counted.values()) * nvox_all
+    b_moved = traffic if traffic is not None else b_counted
+    achieved = b_moved / (launch_us * 1e-6) / 1e9
+    achieved_survey = b_survey / (launch_us * 1e-6) / 1e9
+    # Issue-side roofline for the launches whose busiest unit is the warp schedulers: warp instructions per launch
+    # (the variant's ncu row) / measured launch time / (SMs x 4 schedulers x the SM clock sampled during this run);
+    # one warp instruction per scheduler and clock is the limit.
+    clk_now = clk.summary()
+    n_sm = int(torch.cuda.get_device_properties(dev).multi_processor_count)
+    warp_inst = NCU_ROWS.get(vkey, (None, None, None))[1]
+    issue = None
+    if warp_inst is not None and clk_now.get("sm_mhz"):
+        issue_peak = n_sm * 4 * float(clk_now["sm_mhz"]) * 1e6
+        issue_ach = warp_inst / (launch_us * 1e-6)
+        issue = {"achieved": issue_ach / 1e9, "peak": issue_peak / 1e9, "unit": "G warp-instructions/s",
+                 "frac": issue_ach / issue_peak, "warp_instructions_per_launch": warp_inst,
+                 "warp_instructions_source": NCU_ROWS[vkey][2] + " (smsp__inst_executed.sum)",
+                 "peak_source": "%d SMs x 4 schedulers x %.0f MHz (SM clock sampled during the timed region, NVML), "
+                                "1 warp instruction per scheduler and clock" % (n_sm, float(clk_now["sm_mhz"]))}
     roofline = {
         # S = 1: one pass over the field per step, the HBM stream binds.  S >= 2: the kernel moves the same bytes per
         # launch but does S steps of arithmetic on them; ncu shows the issue slots, not DRAM, as the busiest unit
         # (profiles/): frac stays the true share of the HBM peak, it is just not what limits the kernel
         "bound": "hbm" if (not blocked or S == 1) else "issue",      # (the one-step kernels, blocked S = 1 or TMA-staged: HBM)
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "bytes_basis": ("DRAM bytes per launch of this variant's ncu capture (traffic_source)" if traffic is not None else
+                        "this build's count: 9 B per voxel + 4 B for the hot share of rows (no ncu capture of this variant)"),
+        "bytes_per_launch": b_moved, "bytes_per_voxel_counted": bytes_counted,
+        "achieved_survey_10B": achieved_survey, "frac_survey_10B": achieved_survey / peak,
         "traffic": traffic, "traffic_source": traffic_src, "variant": vkey, "peak_source": peak_src,
+        "issue": issue,
         "kernel": f"rfa_blocked_kernel<S={S}>" if blocked else ("rfa_stream_kernel (TMA, S=1)" if stream_k else "rfa_plain_kernel"),
         "launches": launches, "full_launches": n_main, "avg_launch_us": launch_us,
         "remainder_launch": {"steps": k_rem, "us": (ms_local - ms_main) * 1e3} if k_rem else None,
@@ -533,7 +572,12 @@ def run_record(args):
         sim.close()
     peak, peak_src = measured_peak()
     fps_rec, fps_hand = K / (ms_rec * 1e-3), K / (ms_hand * 1e-3)
-    b_step = sum(BYTES_SURVEY.values()) * w.n_voxels
+    # the TMA-staged one-step kernel moves 8.48 B per voxel (569.1 MB per C4 launch, profiles/r2_variants_final_ncu.md);
+    # without a capture of the workload: 9 B (theta read + write, state byte).  SURVEY's 10 B is kept as frac_survey_10B.
+    stream_used = q1["kernel"] == binding.KERNEL_STREAM      # what rfa_query reports for one-step launches of this simulation
+    tr = NCU_TRAFFIC.get("C4/S1/128x16/hc%d/eq12/tma" % variant.get("held_copy", 0)) if (w.name == "C4" and stream_used) else None
+    b_step = tr[0] if tr else 9.0 * w.n_voxels
+    b_step_survey = sum(BYTES_SURVEY.values()) * w.n_voxels
     ach = b_step * fps_rec / 1e9
     print(json.dumps({
         "metric": "frames/s (Alg. 2 frame loop: one time step per frame, probes recorded every frame)",
@@ -547,8 +591,11 @@ def run_record(args):
                     "consumer": "device-to-device copy of the finished image (%d MiB) on a second stream, overlapped with "
                                 "the next step" % (nbytes >> 20)},
         "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                     "peak_source": peak_src, "kernel": "rfa_blocked_kernel<S=1> + rfa_probe_kernel",
-                     "algorithmic_bytes_per_launch": b_step, "bytes_per_voxel": BYTES_SURVEY,
+                     "peak_source": peak_src,
+                     "kernel": ("rfa_stream_kernel (TMA, S=1)" if stream_used else "rfa_blocked_kernel<S=1>") + " + rfa_probe_kernel",
+                     "bytes_per_launch": b_step, "bytes_basis": (tr[1] + " (DRAM bytes of the one-step kernel)") if tr else "this build's count: 9 B per voxel",
+                     "algorithmic_bytes_per_launch": b_step_survey, "bytes_per_voxel": BYTES_SURVEY,
+                     "frac_survey_10B": b_step_survey * fps_rec / 1e9 / peak,
                      "equiv_8B_frac": w.n_voxels * fps_rec * 8.0 / 1e9 / peak},
         "gpu_launches": q1["kernel_launches"] - q0["kernel_launches"], "clocks": clk.summary(),
         "check": {"probe_t_c_last_frame": [float(x) for x in last]}}), flush=True)
