@@ -591,7 +591,7 @@ def test_warp_matches_oracle_elementwise(rfa, oracle):
 
 
 def test_warp_full_size_sampled(rfa):
-    """C4 size: sampled voxels against the oracle (it evaluates voxel by voxel), bounds everywhere."""
+    """C4 size: sampled voxels near the needle first (a quick, pointed failure), then the whole field against the oracle."""
     from oracle import rfa_warp_oracle as WO
     w = W.c4_body(steps=300)
     sim = rfa.from_workload(w)
@@ -611,6 +611,15 @@ def test_warp_full_size_sampled(rfa):
     assert float(np.max(np.abs(got.ravel()[idx].astype(np.float64) - exp))) <= TOL
     assert got.min() >= T.min() and got.max() <= T.max()
     assert float(np.abs(got - T).max()) > 1.0                # the heat zone really moved
+    # and EVERY voxel of the 67 M: the oracle is vectorised numpy, fed 16 z planes at a time through its `index` path
+    worst = 0.0
+    gflat = got.ravel()
+    for k0 in range(0, nz, 16):
+        sl = np.arange(k0 * nx * ny, min(k0 + 16, nz) * nx * ny, dtype=np.int64)
+        e = WO.warp_temperature(T, d, np.float32(0.85), w.spacing_mm, index=sl)
+        worst = max(worst, float(np.max(np.abs(gflat[sl].astype(np.float64) - e))))
+    assert worst <= TOL, f"warp, whole field: max |dT| = {worst:.3e}"
+    print(f"warp C4: field max|dT| {worst:.2e} over all {got.size} voxels")
     sim.close()
 
 
@@ -705,6 +714,13 @@ def test_boundary_validation_on_a_live_simulation(rfa):
     with pytest.raises(ValueError):
         sim.step_record(4, 2, out=np.empty((2, 2), np.float32))
     sim.close()
+    # a label id outside the tissue table is found by the device histogram of rfa_create (no host walk when a device is there)
+    wbad = W.ragged_phantom(dims=(44, 38, 29), spacing=(1.0, 1.0, 1.0), steps=5)
+    wbad.labels = wbad.labels.copy()
+    wbad.labels[7, 11, 13] = len(wbad.table)
+    with pytest.raises(rfa.RfaError) as ei:
+        rfa.from_workload(wbad)
+    assert ei.value.code == rfa.RFA_E_INVALID and "label" in str(ei.value)
     # a forced tile shape that cannot run is refused under every kernel setting but PLAIN (nx % 4 != 0: no blocked plan)
     sim = rfa.from_workload(W.ragged_phantom(dims=(45, 38, 29), spacing=(0.7, 0.9, 1.3), steps=3))
     for shape in (0, 1):
@@ -797,7 +813,7 @@ def test_full_length_config_vs_golden(rfa, name):
     sim.close()
 
 
-def test_c4_conservative_conduction_vs_golden(rfa):
+def test_c4_conservative_conduction_vs_golden(rfa, oracle):
     """Row f1 at the full C4 size, in the default launch configuration: sampled voxels (needle region, uniform,
     tissue interfaces) at three checkpoints and the crop at the needle against the conservative fp64 oracle."""
     g = _golden("C4F")
@@ -821,8 +837,14 @@ def test_c4_conservative_conduction_vs_golden(rfa):
     idx = g["sample_idx"]
     assert float(np.max(np.abs(T2.ravel()[idx].astype(np.float64) - g["sample_T"][-1]))) > 0.05
     print(f"C4F: sampled max|dT| {err_s:.2e}, crop {err:.2e}, necrosis mismatches {n_mism}")
-    sim.close()
     sim2.close()
+    # field-wide: every voxel of this workload moves (non-uniform start), so a compact stored field would be the whole
+    # 268 MB image; the conservative oracle runs the 400 steps here instead and all 67 M voxels are compared
+    osim = oracle.run_workload(w, steps=done, conservative=True)
+    assert float(np.max(np.abs(osim.T.ravel()[idx] - g["sample_T"][-1]))) <= 1e-12      # the live oracle reproduces the stored one
+    err_f, n_band = compare(T, N, osim)
+    print(f"C4F: field max|dT| {err_f:.2e} over all {T.size} voxels, {n_band} necrosis differences inside the band")
+    sim.close()
 
 
 def test_c5_sweep_vs_golden(rfa):
@@ -845,13 +867,15 @@ def test_c5_sweep_vs_golden(rfa):
 
 
 def test_c5_sweep_fieldwide_vs_live_oracle(rfa, oracle):
-    """Field-wide on the planning sweep: four seeded scenarios of the 64 are run by the oracle here (3000 steps of
-    128^3 each) and compared voxel by voxel with the batched launch bench.py times (all 64 scenarios in flight)."""
+    """Field-wide on the planning sweep: sixteen seeded scenarios of the 64 are run by the oracle here (3000 steps of
+    128^3 each) and compared voxel by voxel with the batched launch bench.py times (all 64 scenarios in flight); the
+    other scenarios are covered by test_c5_sweep_vs_golden (samples, crop, full necrosis mask).  A stored compact field
+    for all 64 would be 35 MB of goldens."""
     w = W.c5_sweep()
     sim = rfa.from_workload(w)
     sim.step(w.steps)
     rng = np.random.default_rng(190705709)
-    for b in sorted(rng.choice(w.batch, size=4, replace=False).tolist()):
+    for b in sorted(rng.choice(w.batch, size=16, replace=False).tolist()):
         osim = oracle.run_workload(w, scenario=b)
         err, n_band = compare(sim.get_temperature(b), sim.get_necrosis(b), osim)
         print(f"C5 scenario {b}: field max|dT| {err:.2e}, {n_band} necrosis differences inside the band")
@@ -900,6 +924,34 @@ def test_full_size_short_run_fieldwide_vs_live_oracle(rfa, oracle, name, conserv
     err, n_band = compare(sim.get_temperature(0), sim.get_necrosis(0), osim)
     print(f"{name}{' (conservative)' if conservative else ''}: 7 steps, field max|dT| {err:.2e} over {w.n_voxels} voxels")
     sim.close()
+
+
+@pytest.mark.parametrize("name", ["C4", "C3"])
+def test_full_length_default_configuration_is_bit_identical_to_plain(rfa, name):
+    """The whole configured run (C4: 12 000 steps, C3: 24 000) in the default launch configuration against the
+    one-thread-per-voxel kernel (no tiles, no rings, no barriers, one step per launch), field and mask bit for bit.
+    Only a run of this length gets the residual-prefetch variant switched on by the library's own feedback in mid-run
+    (C3) and work items that are mostly hot; a stale read of a shared-memory ring slot or of a halo plane anywhere in
+    those launches would show here, which stands in for the racecheck run this pool does not allow."""
+    w = W.BENCH_CONFIGS[name]()
+    ref = rfa.from_workload(w)
+    ref.configure(rfa.KERNEL_PLAIN, 0)
+    ref.step(w.steps)
+    Tp, Np = ref.get_temperature(0), ref.get_necrosis(0)
+    ref.close()
+    sim = rfa.from_workload(w)
+    for _ in range(8):                          # several calls, as the residual-prefetch test does: the feedback is acted on at launches
+        sim.step(w.steps // 8)
+    hot = sim.hot_fraction()
+    T, N = sim.get_temperature(0), sim.get_necrosis(0)
+    v = sim.query_variant()
+    sim.close()
+    assert v["fused_steps"] == 3 and w.steps % 8 == 0
+    assert np.array_equal(T.view(np.uint32), Tp.view(np.uint32)), f"{name}: default configuration differs from the plain kernel after {w.steps} steps"
+    assert np.array_equal(N, Np)
+    if name == "C3":                            # the umbrella needle warms enough of the volume: the variant switched on by itself
+        assert hot["residual_prefetch"] == 1 and hot["hot_fraction"] >= 0.004, hot      # RFA_HOT_ON
+    print(f"{name}: {w.steps} steps, default configuration == plain kernel bit for bit; hot fraction {hot}")
 
 
 def test_residual_prefetch_switches_on_by_itself(rfa):
