@@ -51,26 +51,30 @@ BYTES_BUILD = {"theta_read": 4.0, "theta_write": 4.0, "state_byte_read": 1.0, "r
 # dram__bytes_write.sum) and warp instructions executed (smsp__inst_executed.sum).  Keyed by the variant string of the run
 # (workload / fused steps / tile / held-copy / conduction / staging / residual prefetch): a run whose variant has no row
 # prints "traffic": null and "issue": null.
-_V = "profiles/r2_variants_final_ncu.md"
+_V = "profiles/r3_variants_ncu.md"
 _AB = "profiles/r2_blocked_ab_ncu.md"
 NCU_ROWS = {
     # variant: (DRAM bytes per launch, warp instructions per launch or None, profile file)
-    "C4/S3/64x32/hc1/eq12": (588.4e6, 147.27e6, "profiles/r2_blocked_s3_final_ncu.md"),
-    "C4/S3/64x32/hc0/eq12": (577.4e6, 164.02e6, _V),
-    "C4/S3/64x32/hc1/eq12/tma": (592.5e6, 154.73e6, _V),
-    "C4/S2/64x32/hc1/eq12": (577.5e6, 89.80e6, _V),
-    "C4/S4/64x32/hc1/eq12": (580.2e6, 198.97e6, _V),
-    "C4/S1/64x32/hc1/eq12": (578.0e6, 47.44e6, _V),
-    "C4/S1/128x16/hc1/eq12/tma": (568.9e6, 50.86e6, _V),
+    "C4/S3/64x32/hc1/eq12": (588.2e6, 145.79e6, _V),
+    "C4/S3/64x32/hc0/eq12": (577.1e6, 164.02e6, _V),
+    "C4/S3/64x32/hc1/eq12/tma": (593.6e6, 153.31e6, _V),
+    "C4/S2/64x32/hc1/eq12": (576.9e6, 88.84e6, _V),
+    "C4/S4/64x32/hc1/eq12": (580.0e6, 197.87e6, _V),
+    "C4/S1/64x32/hc1/eq12": (578.0e6, 46.66e6, _V),
+    "C4/S1/128x16/hc1/eq12/tma": (569.1e6, 50.74e6, _V),
     "C4/S1/128x16/hc0/eq12/tma": (569.3e6, 57.81e6, _V),
+    "C3/S3/64x32/hc0/eq12": (119.6e6, 46.51e6, _V),
+    "C3/S1/128x16/hc0/eq12/tma": (113.4e6, 15.30e6, _V),
+    "C5/S2/128x16/hc0/eq12/tma": (1199.9e6, 220.86e6, _V),
+    "C5/S3/128x16/hc0/eq12/tma": (1186.2e6, 367.37e6, _V),
+    "C2/S2/128x16/hc0/eq12/tma": (10.6e6, 6.26e6, _V),
+    "C1/S3/64x32/hc0/eq12": (1.4e6, 4.43e6, _V),
+    "C4/S3/64x32/hc1/face": (642.0e6, 180.77e6, _V),
+    "C4F/S3/64x32/hc1/face": (851.2e6, 344.96e6, _V),
+    "C4/plain": (840.3e6, 494.93e6, _V),
+    # after ~2700 steps (hot region grown, residual prefetch on): rows of profiles/r2_blocked_ab_ncu.md, no instruction count there
     "C3/S3/64x32/hc0/eq12/rpf": (120.6e6, None, _AB),
-    "C3/S3/64x32/hc0/eq12": (119.0e6, 46.51e6, _V),
-    "C5/S2/128x16/hc0/eq12/tma": (1200.2e6, 220.86e6, _V),
-    "C5/S3/128x16/hc0/eq12/tma": (1185.6e6, 367.36e6, _V),
-    "C4/S3/64x32/hc1/face": (642.4e6, 182.25e6, _V),
-    "C4F/S3/64x32/hc1/face": (855.0e6, 345.18e6, _V),
     "C4F/S3/64x32/hc1/face/rpf": (870.9e6, None, _AB),
-    "C4/plain": (840.6e6, 494.93e6, _V),
 }
 NCU_TRAFFIC = {k: (v[0], v[2]) for k, v in NCU_ROWS.items()}
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
@@ -259,6 +263,33 @@ def pinned(a):
     return t, v
 
 
+def measure_l2_and_launch_floor(dev, stream):
+    """Two measured denominators for volumes that never leave the 126 MB L2 (C1, C2), where an HBM fraction says nothing:
+      l2_copy_gbs      read + write bytes per second of `b.copy_(a)` between two 16 MiB device buffers, 200 copies back to
+                       back on the bench stream (both buffers stay in L2 after the first copy), CUDA events
+      launch_floor_us  time per launch of 400 back-to-back 4-byte copies on the same stream: what a launch costs when
+                       the kernel does nothing (the floor under any one-launch-per-few-steps scheme)"""
+    import torch
+    a = torch.empty(4 << 20, dtype=torch.float32, device=dev)
+    b = torch.empty_like(a)
+    t = torch.zeros(1, dtype=torch.float32, device=dev)
+    u = torch.zeros(1, dtype=torch.float32, device=dev)
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    with torch.cuda.stream(stream):
+        for _ in range(10):
+            b.copy_(a)
+            u.copy_(t)
+        e0.record(stream)
+        for _ in range(200):
+            b.copy_(a)
+        e1.record(stream)
+        for _ in range(400):
+            u.copy_(t)
+        e2.record(stream)
+        e2.synchronize()
+    return 2.0 * a.numel() * 4 * 200 / (e0.elapsed_time(e1) * 1e-3) / 1e9, e1.elapsed_time(e2) * 1e3 / 400
+
+
 def run_ours(args):
     import torch
     from paper_1907_05709_b200 import binding, workloads as W
@@ -397,6 +428,22 @@ def run_ours(args):
         "equiv_8B_frac": gvox / world * 8.0 / peak,
     }
 
+    fits_l2 = nvox_all * 9 <= 126e6              # the same test as config.l2 below: what one step touches (2 fields + state) vs the 126 MB L2
+    if fits_l2 and world == 1:
+        # the volume stays in L2 from launch to launch: report against a measured L2 copy rate and the launch floor,
+        # and keep the HBM share only as a labelled side figure
+        l2_gbs, floor_us = measure_l2_and_launch_floor(dev, stream)
+        achieved = b_counted / (launch_us * 1e-6) / 1e9      # bytes through L2 (this build's count), not the DRAM trickle
+        roofline.update({
+            "bound": "l2+launch", "achieved": achieved, "peak": l2_gbs, "frac": achieved / l2_gbs,
+            "bytes_per_launch": b_counted, "bytes_basis": "this build's count through L2: 9 B per voxel + 4 B for the hot share of rows "
+                                                          "(the DRAM traffic of an L2-resident volume, `traffic`, is next to nothing)",
+            "peak_source": "measured here: torch b.copy_(a) between two 16 MiB device buffers, 200 copies back to back (L2-resident), read + write bytes; a 6 us copy kernel carries its own launch and tail overhead, so this is a floor of the L2 rate and frac an upper estimate",
+            "frac_of_hbm_copy_peak": achieved / peak, "hbm_copy_peak": peak,
+            "launch_floor_us": floor_us, "launch_floor_frac": floor_us / launch_us,
+            "launch_floor_source": "measured here: 400 back-to-back 4-byte device copies on the bench stream, time per launch",
+        })
+
     # ---- end-to-end leg: host buffers in, host buffers out --------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -404,36 +451,42 @@ def run_ours(args):
         masks = [pinned(np.ascontiguousarray(nd.mask, dtype=np.uint8))[1] for nd in w.needles]
         _, T_h = pinned(np.empty((nz, ny, nx), np.float32))
         _, N_h = pinned(np.empty((nz, ny, nx), np.uint8))
-        torch.cuda.synchronize(dev)
-        if dist is not None:
-            dist.barrier()
-        t0 = time.perf_counter()
-        with torch.cuda.stream(stream):
-            s2 = binding.RfaSim(w.dims, w.spacing_mm, lab_h, w.table, w.t_blood, w.dt, batch=w.batch,
-                                device=dev, stream=stream)
-            s2.configure(args.kernel, args.fused)
-            if hc_env in ("0", "1"):
-                s2.configure_held_copy(int(hc_env))
-            if args.conduction == "face":
-                s2.set_conduction(binding.COND_FACE)
-            for b, nd in enumerate(w.needles):
-                s2.set_needle(b, masks[b], nd.mode, nd.value, nd.tip_mm, nd.axis)
-            s2.step(K)
-            for b in range(w.batch):
-                s2.get_temperature(b, out=T_h)
-                s2.get_necrosis(b, out=N_h)
-            s2.synchronize()
-        torch.cuda.synchronize(dev)
-        e2e_ms_local = (time.perf_counter() - t0) * 1e3
-        s2.close()
+        # The whole job three times, each through the public API from host buffers to host buffers; the MEDIAN is reported
+        # and all three are listed.  A single shot is at the mercy of one cudaMalloc of the 0.7 GB workspace, which on a
+        # fresh process takes anything between 1 and 25 ms (measured: jobs of 12.9 / 18.2 / 39.0 ms for the same 20 steps).
+        e2e_runs = []
+        for _rep in range(3):
+            torch.cuda.synchronize(dev)
+            if dist is not None:
+                dist.barrier()
+            t0 = time.perf_counter()
+            with torch.cuda.stream(stream):
+                s2 = binding.RfaSim(w.dims, w.spacing_mm, lab_h, w.table, w.t_blood, w.dt, batch=w.batch,
+                                    device=dev, stream=stream)
+                s2.configure(args.kernel, args.fused)
+                if hc_env in ("0", "1"):
+                    s2.configure_held_copy(int(hc_env))
+                if args.conduction == "face":
+                    s2.set_conduction(binding.COND_FACE)
+                for b, nd in enumerate(w.needles):
+                    s2.set_needle(b, masks[b], nd.mode, nd.value, nd.tip_mm, nd.axis)
+                s2.step(K)
+                for b in range(w.batch):
+                    s2.get_temperature(b, out=T_h)
+                    s2.get_necrosis(b, out=N_h)
+                s2.synchronize()
+            torch.cuda.synchronize(dev)
+            e2e_runs.append((time.perf_counter() - t0) * 1e3)
+            s2.close()
+        e2e_ms_local = float(np.median(e2e_runs))
         e2e_ms, e2e_units = aggregate(e2e_ms_local, float(nvox_all) * K, dist, dev)
         h2d = w.n_voxels * (1 + len(w.needles))
         d2h = w.n_voxels * 5 * w.batch
         e2e = {"value": e2e_units / (e2e_ms * 1e-3) / 1e9, "unit": METRIC,
                "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
-               "h2d_bytes_per_job": h2d, "d2h_bytes_per_job": d2h, "job_ms": e2e_ms,
+               "h2d_bytes_per_job": h2d, "d2h_bytes_per_job": d2h, "job_ms": e2e_ms, "job_ms_runs": e2e_runs,
                "what": "rfa_create(host labels) + rfa_set_needle(host mask) + rfa_step(K) + rfa_get_temperature/"
-                       "rfa_get_necrosis into pinned host buffers, host clock, allocation included"}
+                       "rfa_get_necrosis into pinned host buffers, host clock, allocation included; median of 3 whole jobs"}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -447,7 +500,7 @@ def run_ours(args):
             "config": {"workload": w.name, "dims": [nx, ny, nz], "batch": w.batch, "spacing_mm": list(w.spacing_mm),
                        "dt_s": w.dt, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2 (2 x %d MiB fields + %d MiB state vs 126 MB L2)" % (
-                           nvox_all * 4 >> 20, nvox_all >> 20) if nvox_all * 9 > 126e6 * 2 else
+                           nvox_all * 4 >> 20, nvox_all >> 20) if nvox_all * 9 > 126e6 else
                              "working set fits L2 (reported, not held to the HBM bar)",
                        "kernel": roofline["kernel"], "conduction": args.conduction, "variant": variant},
             "sim_steps_per_s": K / (ms * 1e-3) * (1 if world == 1 else world),
@@ -572,7 +625,7 @@ def run_record(args):
         sim.close()
     peak, peak_src = measured_peak()
     fps_rec, fps_hand = K / (ms_rec * 1e-3), K / (ms_hand * 1e-3)
-    # the TMA-staged one-step kernel moves 8.48 B per voxel (569.1 MB per C4 launch, profiles/r2_variants_final_ncu.md);
+    # the TMA-staged one-step kernel moves 8.48 B per voxel (569.1 MB per C4 launch, profiles/r3_variants_ncu.md);
     # without a capture of the workload: 9 B (theta read + write, state byte).  SURVEY's 10 B is kept as frac_survey_10B.
     stream_used = q1["kernel"] == binding.KERNEL_STREAM      # what rfa_query reports for one-step launches of this simulation
     tr = NCU_TRAFFIC.get("C4/S1/128x16/hc%d/eq12/tma" % variant.get("held_copy", 0)) if (w.name == "C4" and stream_used) else None
